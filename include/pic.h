@@ -1,0 +1,177 @@
+/* pic.h — C ABI of the B200-native electromagnetic PIC step (libpic.so).
+ *
+ * One call sequence runs the per-step particle loop of the electromagnetic PIC method that
+ * arXiv 2101.12149 ("Porting WarpX to GPU-accelerated platforms") ports to GPUs:
+ *   cell-tile particle sort      (§3.4.2 "Particle Sorting")
+ *   fused field gather + push    (§3.1: fields re-gathered inside the push kernel)
+ *   Esirkepov current deposition (§3.4.1; ref [8] PAPER.md:301)
+ *   Yee FDTD update of E and B   (§2.4: B on faces, E and J on edges; ref [28])
+ *   guard-cell sum and fill      (§2.4 FillBoundary / SumBoundary)
+ * on ONE GPU, one periodic (or z-truncated) box. The formulas are fixed in DESIGN.md
+ * ("The step", "Readings"); every step runs in hand-written CUDA kernels for sm_100a.
+ * There is no CPU fallback: every call fails with PIC_ERR_CUDA when no device is usable.
+ *
+ * Conventions
+ *  - Units: SI. Positions in metres inside [0, n_cells[d]*dx[d]); momenta u = gamma*v in m/s;
+ *    weight = real particles per macro-particle; E in V/m, B in T, J in A/m^2.
+ *  - Element type of every `void*` array is double under PIC_F64 and float under PIC_F32.
+ *  - Fields: one array per component holding n_x*n_y*n_z values of the valid region, x fastest
+ *    (idx = i + n_x*(j + n_y*k), "Fortran index order"); guard cells are internal.
+ *    Array element [i,j,k] of a component is the value at its Yee location:
+ *      Ex,Jx (i+1/2,j,k)  Ey,Jy (i,j+1/2,k)  Ez,Jz (i,j,k+1/2)
+ *      Bx (i,j+1/2,k+1/2) By (i+1/2,j,k+1/2) Bz (i+1/2,j+1/2,k)
+ *  - Particles: structure of arrays, one array per attribute.
+ *  - `where` says whether the caller's pointers are host (PIC_HOST) or device (PIC_DEVICE)
+ *    memory. The library copies every input during the call (the caller may free at once) and
+ *    writes outputs into caller-allocated buffers. Scalars and small structs are host memory.
+ *  - Time levels: supplied u is u^{n-1/2}; supplied x, E, B are at time n. No back-push.
+ *  - Every call returns 0 or a negative PIC_ERR_*; nothing throws or aborts across the ABI.
+ *    pic_step is asynchronous on the simulation's stream; asynchronous faults surface at the
+ *    next synchronising call (pic_get_*, pic_synchronize).
+ *  - A pic_sim is not thread-safe; use one host thread per handle.
+ */
+#ifndef PIC_H_
+#define PIC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define PIC_API __attribute__((visibility("default")))
+#else
+#define PIC_API
+#endif
+
+typedef struct pic_sim pic_sim; /* opaque; created by pic_create, freed by pic_destroy */
+
+typedef enum { PIC_F64 = 0, PIC_F32 = 1 } pic_precision;
+typedef enum { PIC_HOST = 0, PIC_DEVICE = 1 } pic_mem;
+
+enum {
+  PIC_OK = 0,
+  PIC_ERR_INVALID_ARG = -1,   /* null pointer, order not in 1..3, tile does not divide, n < 0, NaN/Inf input */
+  PIC_ERR_CFL = -2,           /* dt*c*sqrt(sum 1/dx^2) > 1 */
+  PIC_ERR_OUT_OF_DOMAIN = -3, /* a particle position outside [0, L) */
+  PIC_ERR_OOM = -4,           /* device allocation failed */
+  PIC_ERR_CUDA = -5,          /* CUDA error (text in pic_last_error), or no CUDA device */
+  PIC_ERR_CAPACITY = -6       /* caller's output buffer too small */
+};
+
+/* Deposition kernels: all compute the same sums in a different order. */
+enum {
+  PIC_DEPOSIT_AUTO = 0,       /* library's choice for the precision / order / sort state */
+  PIC_DEPOSIT_GLOBAL = 1,     /* one thread per particle, one global atomic per particle-node
+                                 (the paper's GPU design) */
+  PIC_DEPOSIT_COOP = 2        /* warp-cooperative: a warp walks its particles, lanes own window
+                                 nodes, sums held in registers per cell run, one flush per run */
+};
+
+/* Options; pass NULL to pic_create for the defaults given here. */
+typedef struct {
+  int32_t periodic[3];   /* default {1,1,1}; 0 = truncation with zeroed guard cells on that axis:
+                            fields outside read 0, J deposited outside is dropped, a particle
+                            leaving through it is deactivated (weight := 0) */
+  int32_t tile[3];       /* cells per sort tile, default {8,8,8}; each must divide n_cells (a tile
+                            larger than the grid is clipped to the grid) */
+  int32_t sort_interval; /* sort every this many steps, first at step 0; default 4
+                            (PAPER.md:201); 0 = never */
+  int32_t sort_key_mode; /* 0 = tile-major cell key (default): tile index major, cell inside
+                            the tile minor; 1 = tile index only */
+  int32_t deposit_mode;  /* PIC_DEPOSIT_*; default PIC_DEPOSIT_AUTO */
+  int32_t reserved;      /* must be 0 */
+  void*   cuda_stream;   /* cudaStream_t all work is issued on (e.g. torch's current stream);
+                            NULL = the legacy default stream */
+} pic_options;
+
+/* Fill *opt with the defaults. */
+PIC_API void pic_default_options(pic_options* opt);
+
+/* Create a simulation on the current CUDA device: a box of n_cells[3] Yee cells of size dx[3]
+ * (metres), time step dt (seconds), B-spline shape order 1..3 used for both gather and deposit,
+ * working precision prec. Fields start at zero. *out receives the handle.
+ * Errors: INVALID_ARG, CFL, OOM, CUDA. */
+PIC_API int pic_create(const int32_t n_cells[3], const double dx[3], double dt, int shape_order,
+               pic_precision prec, const pic_options* opt, pic_sim** out);
+
+/* Add a species of n macro-particles (one container per species) with charge (C)
+ * and mass (kg) per real particle. x..w are arrays of n elements in `where` memory. Particle ids
+ * are 0..n-1 in the order given and follow the particles through every sort. *species_id
+ * (nullable) receives the species index (0,1,...). Species are processed in insertion order.
+ * Errors: INVALID_ARG (incl. non-finite values), OUT_OF_DOMAIN, OOM, CUDA. Synchronises. */
+PIC_API int pic_add_species(pic_sim* sim, int64_t n, const void* x, const void* y, const void* z,
+                    const void* ux, const void* uy, const void* uz, const void* w,
+                    double charge, double mass, pic_mem where, int32_t* species_id);
+
+/* Overwrite E and B (valid region, layout above) and refresh the guard cells. E, B: arrays of
+ * three pointers. Errors: INVALID_ARG (incl. non-finite), CUDA. Synchronises. */
+PIC_API int pic_set_fields(pic_sim* sim, const void* const E[3], const void* const B[3], pic_mem where);
+
+/* Advance n steps: per step, per species { sort if due } -> zero J -> per species
+ * { gather + Boris push + Esirkepov deposit + wrap } -> sum J guards -> B half step -> E full
+ * step -> B half step -> fill E/B guards. Asynchronous. */
+PIC_API int pic_step(pic_sim* sim, int32_t n);
+
+/* Block until all issued work is done; returns PIC_ERR_CUDA if any of it faulted. */
+PIC_API int pic_synchronize(pic_sim* sim);
+
+/* Copy the valid region of E, B and (if J != NULL) the J of the last step into the caller's
+ * arrays (three pointers each, n_x*n_y*n_z elements). Any of E, B, J may be NULL. Synchronises. */
+PIC_API int pic_get_fields(pic_sim* sim, void* const E[3], void* const B[3], void* const J[3], pic_mem where);
+
+/* Copy species `species` in its CURRENT internal order into caller arrays of `capacity`
+ * elements (any pointer may be NULL to skip that attribute); *n_out (nullable) = particle count.
+ * Errors: INVALID_ARG, CAPACITY. Synchronises. */
+PIC_API int pic_get_particles(pic_sim* sim, int32_t species, int64_t capacity, void* x, void* y, void* z,
+                      void* ux, void* uy, void* uz, void* w, int64_t* id, int64_t* n_out, pic_mem where);
+
+/* State of the most recent sort of a species: cell[k] = linear cell index
+ * (c_x + n_x*(c_y + n_y*c_z)) of the particle in slot k right after that sort, perm[k] = slot
+ * the particle held before it. Either pointer may be NULL. Errors: INVALID_ARG (never sorted). */
+PIC_API int pic_get_sort_state(pic_sim* sim, int32_t species, int32_t* cell, int32_t* perm, pic_mem where);
+
+/* Sort every species now (the same operation pic_step runs when a sort is due). Asynchronous. */
+PIC_API int pic_sort_now(pic_sim* sim);
+
+/* Diagnostics, reduced on the device in fp64 (host array of PIC_NDIAG doubles). Synchronises. */
+enum {
+  PIC_DIAG_FIELD_E = 0,     /* 1/2 eps0 sum E^2 dV  [J] */
+  PIC_DIAG_FIELD_B = 1,     /* 1/2 eps0 c^2 sum B^2 dV [J] */
+  PIC_DIAG_KINETIC = 2,     /* sum w m c^2 (gamma-1) over all species, at the stored u [J] */
+  PIC_DIAG_CHARGE = 3,      /* sum q w [C] */
+  PIC_DIAG_GAUSS_MAX = 4,   /* max |div E - rho/eps0|, rho from the order-n nodal shape */
+  PIC_DIAG_RHO_MAX = 5,     /* max |rho/eps0| */
+  PIC_DIAG_DEACTIVATED = 6, /* particles deactivated at a non-periodic boundary so far */
+  PIC_DIAG_STEPS = 7,       /* steps taken */
+  PIC_DIAG_POOL_CHUNKS = 8, /* cudaMalloc calls made by the memory pool so far */
+  PIC_DIAG_POOL_BYTES = 9,  /* bytes held by the pool */
+  PIC_DIAG_LAUNCHES = 10,   /* kernels launched by this handle so far */
+  PIC_NDIAG = 11
+};
+PIC_API int pic_get_diagnostics(pic_sim* sim, double* out);
+
+/* Nodal charge density rho (C/m^3, fp64, n_x*n_y*n_z, x fastest) of all species. Synchronises. */
+PIC_API int pic_get_rho(pic_sim* sim, double* rho, pic_mem where);
+
+/* Elapsed device time (ms) spent in each phase since the last call with reset != 0; host array
+ * of PIC_NPHASE floats. Phase timing is off until pic_enable_phase_timing(sim, 1). */
+enum { PIC_PHASE_SORT = 0, PIC_PHASE_PARTICLES = 1, PIC_PHASE_FIELDS = 2, PIC_NPHASE = 3 };
+PIC_API int pic_enable_phase_timing(pic_sim* sim, int32_t on);
+PIC_API int pic_get_phase_times(pic_sim* sim, float* ms, int32_t reset);
+
+PIC_API int64_t pic_num_particles(const pic_sim* sim, int32_t species); /* < 0 on error */
+PIC_API int32_t pic_num_species(const pic_sim* sim);
+
+/* Text of the last error of this handle ("" if none). sim == NULL: the last pic_create error.
+ * The string is owned by the library and valid until the next call on the same handle. */
+PIC_API const char* pic_last_error(const pic_sim* sim);
+
+/* Free everything the handle owns (synchronises). NULL is a no-op. */
+PIC_API void pic_destroy(pic_sim* sim);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PIC_H_ */

@@ -1,0 +1,91 @@
+// Shared device-side definitions of the CUDA path (sm_100a). Not used by oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace pic {
+
+// CODATA 2018.
+constexpr double kC = 299792458.0;
+constexpr double kEps0 = 8.8541878128e-12;
+
+constexpr int kGuard = 4;  // guard cells per side
+
+// Field storage: every component is a padded box (N+2G)^3, x fastest; (i,j,k) in [-G, N+G).
+template <class R>
+struct Grid {
+  int N[3];
+  int P[3];          // padded extents
+  int sy, sz;        // strides of j and k in elements (sx = 1)
+  int org;           // linear offset of node (0,0,0)
+  int periodic[3];
+  R inv_dx[3], L[3], cB[3], cE[3], cJ, inv_c2, dt;
+  R* F[6];           // Ex Ey Ez Bx By Bz
+  R* J[3];
+  __host__ __device__ __forceinline__ int idx(int i, int j, int k) const { return org + i + sy * j + sz * k; }
+  __host__ __device__ __forceinline__ int64_t padded_total() const { return (int64_t)P[0] * P[1] * P[2]; }
+};
+
+// One species' particle arrays (structure of arrays).
+template <class R>
+struct Particles {
+  R *x, *y, *z, *ux, *uy, *uz, *w;
+  int64_t* id;
+  int64_t n;
+  R kq;      // q*dt/(2m)
+  R jf[3];   // q/(dt*dx_a*dx_b)
+};
+
+struct TileSpec {
+  int T[3];      // cells per tile
+  int nt[3];     // tiles per axis
+  int tvol;      // cells per tile
+  int key_mode;  // 0 tile-major cell key, 1 tile only
+};
+
+// ------------------------------------------------------------------ shape factors
+// B-spline weights of order n at normalised coordinate xi; returns the leftmost node index.
+template <class R, int ORDER>
+__device__ __forceinline__ int shape(R xi, R* w) {
+  if constexpr (ORDER == 1) {
+    R m = floor(xi);
+    R d = xi - m;
+    w[0] = R(1) - d;
+    w[1] = d;
+    return (int)m;
+  } else if constexpr (ORDER == 2) {
+    R m = floor(xi + R(0.5));
+    R d = xi - m;
+    R a = R(0.5) - d, b = R(0.5) + d;
+    w[0] = R(0.5) * a * a;
+    w[1] = R(0.75) - d * d;
+    w[2] = R(0.5) * b * b;
+    return (int)m - 1;
+  } else {
+    R m = floor(xi);
+    R d = xi - m;
+    R e = R(1) - d;
+    const R s = R(1) / R(6);
+    w[0] = e * e * e * s;
+    w[1] = (R(4) - R(6) * d * d + R(3) * d * d * d) * s;
+    w[2] = (R(4) - R(6) * e * e + R(3) * e * e * e) * s;
+    w[3] = d * d * d * s;
+    return (int)m - 1;
+  }
+}
+
+// one rounded multiply, no FMA contraction
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+
+template <class R>
+__device__ __forceinline__ int cell_of(R x, R inv_dx, int N) {
+  int c = (int)floor(mul_rn(x, inv_dx));
+  return min(max(c, 0), N - 1);
+}
+
+// reduction without return value (RED.E.ADD.F64 / .F32 at L2)
+__device__ __forceinline__ void red_add(double* p, double v) { atomicAdd(p, v); }
+__device__ __forceinline__ void red_add(float* p, float v) { atomicAdd(p, v); }
+
+}  // namespace pic

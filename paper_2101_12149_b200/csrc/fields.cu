@@ -1,0 +1,179 @@
+// Yee FDTD update, J guard sum and E/B guard fill (steps 3-5 and the
+// guard rules; PAPER.md:78 Yee staggering, PAPER.md:73-77 FillBoundary / SumBoundary).
+#include "internal.h"
+
+namespace pic {
+
+namespace {
+
+struct Box3 { int lo[3], n[3]; };
+
+// B -= (dt/2) curl E, forward differences, over the box [lo, lo+n)
+template <class R>
+__global__ void __launch_bounds__(256) k_push_B(Grid<R> g, Box3 b) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  int j = blockIdx.y * blockDim.y + threadIdx.y;
+  int k = blockIdx.z;
+  if (i >= b.n[0] || j >= b.n[1]) return;
+  int t = g.idx(b.lo[0] + i, b.lo[1] + j, b.lo[2] + k);
+  const R* __restrict__ Ex = g.F[0];
+  const R* __restrict__ Ey = g.F[1];
+  const R* __restrict__ Ez = g.F[2];
+  R ex = Ex[t], ey = Ey[t], ez = Ez[t];
+  g.F[3][t] -= g.cB[1] * (Ez[t + g.sy] - ez) - g.cB[2] * (Ey[t + g.sz] - ey);
+  g.F[4][t] -= g.cB[2] * (Ex[t + g.sz] - ex) - g.cB[0] * (Ez[t + 1] - ez);
+  g.F[5][t] -= g.cB[0] * (Ey[t + 1] - ey) - g.cB[1] * (Ex[t + g.sy] - ex);
+}
+
+// E += dt (c^2 curl B - J/eps0), backward differences
+template <class R>
+__global__ void __launch_bounds__(256) k_push_E(Grid<R> g, Box3 b) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  int j = blockIdx.y * blockDim.y + threadIdx.y;
+  int k = blockIdx.z;
+  if (i >= b.n[0] || j >= b.n[1]) return;
+  int t = g.idx(b.lo[0] + i, b.lo[1] + j, b.lo[2] + k);
+  const R* __restrict__ Bx = g.F[3];
+  const R* __restrict__ By = g.F[4];
+  const R* __restrict__ Bz = g.F[5];
+  R bx = Bx[t], by = By[t], bz = Bz[t];
+  g.F[0][t] += g.cE[1] * (bz - Bz[t - g.sy]) - g.cE[2] * (by - By[t - g.sz]) - g.cJ * g.J[0][t];
+  g.F[1][t] += g.cE[2] * (bx - Bx[t - g.sz]) - g.cE[0] * (bz - Bz[t - 1]) - g.cJ * g.J[1][t];
+  g.F[2][t] += g.cE[0] * (by - By[t - 1]) - g.cE[1] * (bx - Bx[t - g.sy]) - g.cJ * g.J[2][t];
+}
+
+// SumBoundary on one periodic box: every valid node within G of a periodic face collects its
+// guard images in a fixed order (deterministic, no atomics). Images on a non-periodic axis are
+// dropped. One thread per valid node of the shell; three components per thread.
+template <class R>
+__global__ void __launch_bounds__(256) k_fold_J(Grid<R> g) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  int j = blockIdx.y * blockDim.y + threadIdx.y;
+  int k = blockIdx.z;
+  if (i >= g.N[0] || j >= g.N[1]) return;
+  const int G = kGuard;
+  int c[3] = {i, j, k};
+  int lo[3], hi[3];
+  bool any = false;
+  for (int d = 0; d < 3; ++d) {
+    // image shifts s*N with s in [lo,hi]: c - N >= -G  <=>  c >= N-G (image below); c + N < N+G <=> c < G
+    lo[d] = (g.periodic[d] && c[d] >= g.N[d] - G) ? -1 : 0;
+    hi[d] = (g.periodic[d] && c[d] < G) ? 1 : 0;
+    any |= (lo[d] != 0) | (hi[d] != 0);
+  }
+  if (!any) return;
+  int t = g.idx(i, j, k);
+  for (int comp = 0; comp < 3; ++comp) {
+    R* __restrict__ J = g.J[comp];
+    R acc = J[t];
+    for (int sc = lo[2]; sc <= hi[2]; ++sc)
+      for (int sb = lo[1]; sb <= hi[1]; ++sb)
+        for (int sa = lo[0]; sa <= hi[0]; ++sa) {
+          if (sa == 0 && sb == 0 && sc == 0) continue;
+          acc += J[g.idx(i + sa * g.N[0], j + sb * g.N[1], k + sc * g.N[2])];
+        }
+    J[t] = acc;
+  }
+}
+
+// FillBoundary on one periodic box: guard <- periodic image in the valid region. Guards on a
+// non-periodic axis are left untouched (they hold zeros). Up to 6 arrays per launch.
+template <class R>
+struct ArrList { R* a[6]; int n; };
+
+template <class R>
+__global__ void __launch_bounds__(256) k_fill_guards(Grid<R> g, ArrList<R> arrs) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x - kGuard;
+  int j = blockIdx.y * blockDim.y + threadIdx.y - kGuard;
+  int k = (int)blockIdx.z - kGuard;
+  if (i >= g.N[0] + kGuard || j >= g.N[1] + kGuard) return;
+  int c[3] = {i, j, k};
+  int s[3];
+  bool guard = false;
+  for (int d = 0; d < 3; ++d) {
+    s[d] = c[d];
+    if (c[d] < 0 || c[d] >= g.N[d]) {
+      if (!g.periodic[d]) return;           // zero guard stays zero
+      guard = true;
+      s[d] = c[d] < 0 ? c[d] + g.N[d] : c[d] - g.N[d];
+      if (s[d] < 0 || s[d] >= g.N[d]) return;   // N < G: cannot happen (checked at create)
+    }
+  }
+  if (!guard) return;
+  int dst = g.idx(i, j, k), src = g.idx(s[0], s[1], s[2]);
+  for (int a = 0; a < arrs.n; ++a) arrs.a[a][dst] = arrs.a[a][src];
+}
+
+template <class R>
+__global__ void __launch_bounds__(256) k_pack(Grid<R> g, const R* __restrict__ src, R* __restrict__ dst) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  int j = blockIdx.y * blockDim.y + threadIdx.y;
+  int k = blockIdx.z;
+  if (i >= g.N[0] || j >= g.N[1]) return;
+  dst[g.idx(i, j, k)] = src[(size_t)i + (size_t)g.N[0] * ((size_t)j + (size_t)g.N[1] * k)];
+}
+
+template <class R>
+__global__ void __launch_bounds__(256) k_unpack(Grid<R> g, const R* __restrict__ src, R* __restrict__ dst) {
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  int j = blockIdx.y * blockDim.y + threadIdx.y;
+  int k = blockIdx.z;
+  if (i >= g.N[0] || j >= g.N[1]) return;
+  dst[(size_t)i + (size_t)g.N[0] * ((size_t)j + (size_t)g.N[1] * k)] = src[g.idx(i, j, k)];
+}
+
+inline dim3 blk() { return dim3(64, 4, 1); }
+inline dim3 grd(int nx, int ny, int nz) { return dim3((nx + 63) / 64, (ny + 3) / 4, nz); }
+
+}  // namespace
+
+template <class R>
+void launch_push_B(const Grid<R>& g, const int lo[3], const int hi[3], Ctx& c) {
+  Box3 b;
+  for (int d = 0; d < 3; ++d) { b.lo[d] = lo[d]; b.n[d] = hi[d] - lo[d]; }
+  k_push_B<R><<<grd(b.n[0], b.n[1], b.n[2]), blk(), 0, c.stream>>>(g, b);
+  c.launches++;
+}
+template <class R>
+void launch_push_E(const Grid<R>& g, const int lo[3], const int hi[3], Ctx& c) {
+  Box3 b;
+  for (int d = 0; d < 3; ++d) { b.lo[d] = lo[d]; b.n[d] = hi[d] - lo[d]; }
+  k_push_E<R><<<grd(b.n[0], b.n[1], b.n[2]), blk(), 0, c.stream>>>(g, b);
+  c.launches++;
+}
+template <class R>
+void launch_fold_J(const Grid<R>& g, Ctx& c) {
+  k_fold_J<R><<<grd(g.N[0], g.N[1], g.N[2]), blk(), 0, c.stream>>>(g);
+  c.launches++;
+}
+template <class R>
+void launch_fill_guards(const Grid<R>& g, R* const* arrays, int narr, Ctx& c) {
+  ArrList<R> l;
+  l.n = narr;
+  for (int a = 0; a < 6; ++a) l.a[a] = a < narr ? arrays[a] : nullptr;
+  k_fill_guards<R><<<grd(g.P[0], g.P[1], g.P[2]), blk(), 0, c.stream>>>(g, l);
+  c.launches++;
+}
+template <class R>
+void launch_pack(const Grid<R>& g, const R* src, R* dst, Ctx& c) {
+  k_pack<R><<<grd(g.N[0], g.N[1], g.N[2]), blk(), 0, c.stream>>>(g, src, dst);
+  c.launches++;
+}
+template <class R>
+void launch_unpack(const Grid<R>& g, const R* src, R* dst, Ctx& c) {
+  k_unpack<R><<<grd(g.N[0], g.N[1], g.N[2]), blk(), 0, c.stream>>>(g, src, dst);
+  c.launches++;
+}
+
+#define INST(R)                                                                         \
+  template void launch_push_B<R>(const Grid<R>&, const int*, const int*, Ctx&);         \
+  template void launch_push_E<R>(const Grid<R>&, const int*, const int*, Ctx&);         \
+  template void launch_fold_J<R>(const Grid<R>&, Ctx&);                                 \
+  template void launch_fill_guards<R>(const Grid<R>&, R* const*, int, Ctx&);            \
+  template void launch_pack<R>(const Grid<R>&, const R*, R*, Ctx&);                     \
+  template void launch_unpack<R>(const Grid<R>&, const R*, R*, Ctx&);
+INST(double)
+INST(float)
+#undef INST
+
+}  // namespace pic

@@ -1,0 +1,58 @@
+// Host-side declarations shared by the translation units of libpic.so (CUDA path only).
+#pragma once
+#include "common.cuh"
+
+namespace pic {
+
+struct Ctx {
+  cudaStream_t stream = nullptr;
+  int64_t launches = 0;   // kernels launched through this handle
+};
+
+// ---- fields.cu
+template <class R> void launch_push_B(const Grid<R>& g, const int lo[3], const int hi[3], Ctx& c);
+template <class R> void launch_push_E(const Grid<R>& g, const int lo[3], const int hi[3], Ctx& c);
+template <class R> void launch_fold_J(const Grid<R>& g, Ctx& c);
+template <class R> void launch_fill_guards(const Grid<R>& g, R* const* arrays, int narr, Ctx& c);
+template <class R> void launch_pack(const Grid<R>& g, const R* valid_src, R* padded_dst, Ctx& c);
+template <class R> void launch_unpack(const Grid<R>& g, const R* padded_src, R* valid_dst, Ctx& c);
+
+// ---- particles.cu
+enum { kDepositGlobal = 1, kDepositCoop = 2 };
+template <class R>
+void launch_particles(const Grid<R>& g, const Particles<R>& p, int order, int mode,
+                      unsigned long long* deactivated, Ctx& c);
+
+// ---- sort.cu
+struct SortScratch {
+  uint32_t* keys[2] = {nullptr, nullptr};
+  uint32_t* vals[2] = {nullptr, nullptr};
+  uint32_t* hist = nullptr;       // 256 * nblocks digit histogram
+  uint32_t* scan_tmp = nullptr;   // block sums of the scan (two levels)
+  int64_t cap = 0;                // particles the buffers are sized for
+  int64_t hist_len = 0;
+  int64_t scan_len = 0;
+};
+int64_t sort_chunk();                                  // keys per block of a radix pass
+int64_t sort_hist_len(int64_t n);                      // entries of `hist` for n particles
+int64_t sort_scan_tmp_len(int64_t hist_len);           // entries of `scan_tmp`
+// Stable sort of `cur` by tile-major cell key into `alt`; fills cell[] and perm[].
+template <class R>
+void sort_species(const Grid<R>& g, const TileSpec& t, const Particles<R>& cur, const Particles<R>& alt,
+                  int32_t* cell, int32_t* perm, SortScratch& s, Ctx& c);
+
+// ---- diag.cu
+template <class R>
+void launch_validate_particles(const Grid<R>& g, const Particles<R>& p, int* flags, Ctx& c);
+template <class R>
+void launch_validate_array(const R* a, int64_t n, int* flags, Ctx& c);
+template <class R>
+void launch_field_energy(const Grid<R>& g, double* out2, Ctx& c);              // out2[0]=sum E^2, [1]=sum B^2
+template <class R>
+void launch_particle_sums(const Particles<R>& p, double q, double m, double* out2, Ctx& c);  // KE, charge
+template <class R>
+void launch_rho(const Grid<R>& g, const Particles<R>& p, int order, double q, double* rho, Ctx& c);
+template <class R>
+void launch_gauss(const Grid<R>& g, const double* rho, double* out2, Ctx& c);  // max|divE-rho/eps0|, max|rho/eps0|
+
+}  // namespace pic

@@ -1,0 +1,267 @@
+"""GPU-vs-oracle parity through the C ABI (BASELINE.json north_star): sort permutation and cell
+indices bit-exact; one step from identical state within 1e-12 (fp64) / 1e-5 (fp32) of each array
+family's max |value|; many-step aggregates within 1e-3."""
+import math
+
+import numpy as np
+import pytest
+
+import workloads as W
+from helpers import compare_state, family_err, make_pair
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-12     # north_star: fp64 one step, normalised by max |value|
+TOL32 = 1e-5      # north_star: fp32 one step
+
+
+def small(cfg_name, n_cells, **kw):
+    return W.scaled(W.CONFIGS[cfg_name], n_cells, **kw)
+
+
+# ------------------------------------------------------------------ sort: bit-exact
+@pytest.mark.parametrize("name,n_cells,tile,key_mode", [
+    ("C1", (16, 16, 16), (8, 8, 8), 0),
+    ("C2", (24, 16, 8), (8, 8, 8), 0),        # several tiles, ragged particle tail (24576 = 6 chunks)
+    ("C2", (20, 12, 28), (4, 4, 4), 0),       # non power-of-two grid, 10+ key bits
+    ("C3", (16, 16, 16), (8, 8, 8), 0),       # fp32 positions
+    ("C2", (16, 16, 16), (8, 8, 8), 1),       # tile-only key
+    ("C2", (16, 8, 8), (1, 1, 1), 0),         # the paper's "sort by cell"
+])
+def test_sort_permutation_and_cells_bit_exact(name, n_cells, tile, key_mode):
+    cfg = small(name, n_cells, tile=tile)
+    import oracle
+    import paper_2101_12149_b200 as pic
+    species, _, _ = W.generate(cfg)
+    a = [species[0][1][k] for k in ("x", "y", "z", "ux", "uy", "uz", "w")]
+    kw = dict(tile=tile, sort_interval=4, sort_key_mode=key_mode)
+    o = oracle.Oracle(cfg.n_cells, cfg.dx, cfg.dt, cfg.order, dtype=cfg.np_dtype, **kw)
+    g = pic.Sim(cfg.n_cells, cfg.dx, cfg.dt, cfg.order, dtype=cfg.np_dtype, **kw)
+    o.add_species(*a, -W.Q_E, W.M_E)
+    g.add_species(*a, -W.Q_E, W.M_E)
+    o.sort_now(); g.sort_now()
+    co, po = o.get_sort_state()
+    cg, pg = g.get_sort_state()
+    assert np.array_equal(pg, po)
+    assert np.array_equal(cg, co)
+    qo, qg = o.get_particles(), g.get_particles()
+    for k in ("id", "x", "y", "z", "ux", "uy", "uz", "w"):
+        assert np.array_equal(qo[k], qg[k]), k          # a permutation moves bits, nothing else
+    # sorting again: identity
+    g.sort_now()
+    _, p2 = g.get_sort_state()
+    assert np.array_equal(p2, np.arange(len(p2), dtype=np.int32))
+
+
+def test_sort_edge_positions_and_ragged_sizes():
+    """x = 0, x just below L (may round to cell N -> clamp), every size around a chunk boundary."""
+    import oracle
+    import paper_2101_12149_b200 as pic
+    n, dx = (8, 8, 8), (1e-6, 0.7e-6, 0.3e-6)
+    dt = 0.5 / (W.C_LIGHT * math.sqrt(sum(1 / d ** 2 for d in dx)))
+    for npart in (1, 31, 4095, 4096, 4097, 9000):
+        rng = np.random.default_rng(npart)
+        pos = rng.uniform(0, 1, (3, npart)) * (np.array(n) * np.array(dx))[:, None]
+        pos[:, 0] = 0.0
+        if npart > 2:
+            pos[:, 1] = np.nextafter(np.array(n) * np.array(dx), 0)
+        z = np.zeros(npart)
+        w = np.ones(npart)
+        o = oracle.Oracle(n, dx, dt, 1, tile=(4, 4, 4))
+        g = pic.Sim(n, dx, dt, 1, tile=(4, 4, 4))
+        o.add_species(pos[0], pos[1], pos[2], z, z, z, w, -W.Q_E, W.M_E)
+        g.add_species(pos[0], pos[1], pos[2], z, z, z, w, -W.Q_E, W.M_E)
+        o.sort_now(); g.sort_now()
+        assert all(np.array_equal(a, b) for a, b in zip(o.get_sort_state(), g.get_sort_state()))
+
+
+# ------------------------------------------------------------------ one step from identical state
+@pytest.mark.parametrize("order", [1, 2, 3])
+@pytest.mark.parametrize("mode", [1, 2])
+def test_one_step_fp64(order, mode):
+    cfg = small("C2", (24, 16, 16), order=order, dx=(1.0e-6, 0.8e-6, 0.6e-6))
+    cfg.species[0].sigma = 0.2            # hot: many cell crossings in one step
+    o, g, _ = make_pair(cfg, fields="random", gpu_kwargs=dict(deposit_mode=mode))
+    o.step(1); g.step(1)
+    assert np.array_equal(o.get_sort_state()[1], g.get_sort_state()[1])
+    compare_state(o, g, TOL64)
+
+
+@pytest.mark.parametrize("order", [1, 3])
+@pytest.mark.parametrize("mode", [1, 2])
+def test_one_step_fp32(order, mode):
+    cfg = small("C3", (24, 16, 16), order=order)
+    cfg.species[0].sigma = 0.1
+    o, g, _ = make_pair(cfg, fields="random", gpu_kwargs=dict(deposit_mode=mode))
+    o.step(1); g.step(1)
+    compare_state(o, g, TOL32)
+
+
+def test_one_step_unsorted_order_is_still_correct():
+    """Correctness must not depend on particles being in their tile."""
+    cfg = small("C2", (16, 16, 16), sort_interval=0)
+    cfg.species[0].sigma = 0.2
+    o, g, _ = make_pair(cfg, fields="random")
+    o.step(2); g.step(2)
+    compare_state(o, g, 20 * TOL64)
+
+
+def test_one_step_two_species():
+    cfg = small("C5", (16, 16, 16))
+    o, g, _ = make_pair(cfg, fields="random")
+    o.step(1); g.step(1)
+    compare_state(o, g, TOL64, n_species=2)
+
+
+def test_one_step_nonperiodic_z_with_laser():
+    cfg = small("C4", (16, 16, 160), z_first=128, ramp_cells=16)
+    o, g, _ = make_pair(cfg)
+    assert max(np.max(np.abs(e)) for e in o.get_fields()[0]) > 1e12      # the laser is there
+    o.step(1); g.step(1)
+    compare_state(o, g, TOL64)
+    o.step(3); g.step(3)
+    compare_state(o, g, 20 * TOL64)
+    assert g.diagnostics()["deactivated"] == o.diagnostics()["deactivated"] == 0
+
+
+def test_particles_leaving_a_nonperiodic_axis_are_deactivated():
+    import oracle
+    import paper_2101_12149_b200 as pic
+    n, dx = (8, 8, 8), (1e-6,) * 3
+    dt = 0.9e-6 / (W.C_LIGHT * math.sqrt(3))
+    x = np.array([4e-6, 4e-6, 4e-6]); y = x.copy()
+    z = np.array([0.05e-6, 7.95e-6, 4e-6])
+    uz = np.array([-5.0, 5.0, 0.1]) * W.C_LIGHT
+    zero = np.zeros(3)
+    w = np.full(3, 1e3)
+    sims = []
+    for mk in (oracle.Oracle, pic.Sim):
+        s = mk(n, dx, dt, 2, periodic=(1, 1, 0), tile=(4, 4, 4))
+        s.add_species(x, y, z, zero, zero, uz, w, -W.Q_E, W.M_E)
+        s.step(1)
+        sims.append(s)
+    o, g = sims
+    assert o.diagnostics()["deactivated"] == 2 and g.diagnostics()["deactivated"] == 2
+    compare_state(o, g, TOL64)
+    assert sorted(g.get_particles()["w"]) == [0.0, 0.0, 1e3]
+
+
+def test_field_solver_only_matches_oracle():
+    cfg = small("C2", (12, 20, 8), dx=(1.0e-6, 0.8e-6, 0.5e-6), tile=(4, 4, 4))
+    cfg.species = []
+    o, g, _ = make_pair(cfg, fields="random")
+    o.step(25); g.step(25)
+    Eo, Bo, _ = o.get_fields(); Eg, Bg, _ = g.get_fields()
+    assert family_err(Eg, Eo) < 1e-13 and family_err(Bg, Bo) < 1e-13
+
+
+def test_empty_and_single_particle_species():
+    import oracle
+    import paper_2101_12149_b200 as pic
+    n, dx = (8, 8, 8), (1e-6,) * 3
+    dt = 0.9e-6 / (W.C_LIGHT * math.sqrt(3))
+    e = np.zeros(0)
+    one = lambda v: np.array([v])
+    sims = []
+    for mk in (oracle.Oracle, pic.Sim):
+        s = mk(n, dx, dt, 3, tile=(4, 4, 4))
+        s.add_species(e, e, e, e, e, e, e, -W.Q_E, W.M_E)
+        s.add_species(one(7.99e-6), one(0.0), one(3.3e-6), one(0.3 * W.C_LIGHT), one(-0.2 * W.C_LIGHT), one(0.0),
+                      one(1e6), W.Q_E, W.M_P)
+        s.step(3)
+        sims.append(s)
+    o, g = sims
+    assert g.num_particles(0) == 0 and g.num_particles(1) == 1
+    Eo, Bo, Jo = o.get_fields(); Eg, Bg, Jg = g.get_fields()
+    assert family_err(Jg, Jo) < TOL64 and family_err(Eg, Eo) < TOL64
+    po, pg = o.get_particles(1), g.get_particles(1)
+    assert family_err([pg[k] for k in "xyz"], [po[k] for k in "xyz"]) < TOL64
+
+
+def test_invalid_inputs_are_rejected_on_device():
+    import paper_2101_12149_b200 as pic
+    n, dx = (8, 8, 8), (1e-6,) * 3
+    dt = 0.9e-6 / (W.C_LIGHT * math.sqrt(3))
+    g = pic.Sim(n, dx, dt, 1)
+    z = np.zeros(4); ok = np.full(4, 1e-6)
+    bad = ok.copy(); bad[2] = 8e-6                       # == L: outside [0, L)
+    with pytest.raises(pic.PicError) as e:
+        g.add_species(bad, ok, ok, z, z, z, ok, -W.Q_E, W.M_E)
+    assert e.value.code == -3
+    nan = ok.copy(); nan[1] = np.nan
+    with pytest.raises(pic.PicError) as e:
+        g.add_species(ok, ok, ok, nan, z, z, ok, -W.Q_E, W.M_E)
+    assert e.value.code == -1
+    assert g.num_particles(0) == -1
+    f = [np.zeros((8, 8, 8)) for _ in range(3)]
+    fb = [np.zeros((8, 8, 8)) for _ in range(3)]; fb[1][0, 0, 0] = np.inf
+    with pytest.raises(pic.PicError):
+        g.set_fields(f, fb)
+
+
+# ------------------------------------------------------------------ many steps: aggregates
+def test_C1_twenty_steps_aggregates():
+    """BASELINE.json config 1 in full (16^3, 2 ppc, fp64, order 1, 20 steps)."""
+    cfg = W.CONFIGS["C1"]
+    o, g, _ = make_pair(cfg)
+    d0 = g.diagnostics()
+    o.step(cfg.steps); g.step(cfg.steps)
+    do, dg = o.diagnostics(), g.diagnostics()
+    eo = do["field_E"] + do["field_B"] + do["kinetic"]
+    eg = dg["field_E"] + dg["field_B"] + dg["kinetic"]
+    assert abs(eg - eo) < 1e-3 * eo
+    assert abs(dg["field_E"] - do["field_E"]) < 1e-3 * do["field_E"]
+    assert dg["charge"] == pytest.approx(do["charge"], rel=1e-12) and dg["charge"] == pytest.approx(d0["charge"], rel=1e-12)
+    # Gauss residual (implicit background): constant in time on both sides
+    assert abs(dg["gauss_max"] - d0["gauss_max"]) < 1e-9 * d0["rho_max"]
+    assert abs(dg["gauss_max"] - do["gauss_max"]) < 1e-9 * do["rho_max"]
+    # after 20 steps (5 sorts) match particles by id
+    po, pg = o.get_particles(), g.get_particles()
+    io, ig = np.argsort(po["id"]), np.argsort(pg["id"])
+    for k in ("x", "ux"):
+        assert np.max(np.abs(po[k][io] - pg[k][ig])) < 1e-9 * np.max(np.abs(po[k]))
+
+
+@pytest.mark.parametrize("order", [1, 3])
+def test_plasma_oscillation_frequency_matches_oracle(order):
+    """T9 set-up on both sides: frequency from zero crossings of Ex agrees to 1e-3."""
+    import oracle
+    import paper_2101_12149_b200 as pic
+    n, dx = (16, 4, 4), (1e-6,) * 3
+    dt = 0.99e-6 / (W.C_LIGHT * math.sqrt(3))
+    g1 = (np.arange(2) + 0.5) / 2
+    cx, cy, cz = np.meshgrid(np.arange(n[0]), np.arange(n[1]), np.arange(n[2]), indexing="ij")
+    pts = [((cx + a).ravel(), (cy + b).ravel(), (cz + c).ravel()) for a in g1 for b in g1 for c in g1]
+    x = np.concatenate([p[0] for p in pts]) * 1e-6
+    y = np.concatenate([p[1] for p in pts]) * 1e-6
+    z = np.concatenate([p[2] for p in pts]) * 1e-6
+    ux = 1e-4 * W.C_LIGHT * np.sin(2 * math.pi * x / 16e-6)
+    w = np.full(len(x), 1e24 * 1e-18 / 8)
+    freqs = []
+    for mk in (oracle.Oracle, pic.Sim):
+        s = mk(n, dx, dt, order, tile=(4, 4, 4), sort_interval=4)
+        s.add_species(x, y, z, ux, 0 * x, 0 * x, w, -W.Q_E, W.M_E)
+        tr = []
+        for _ in range(300):
+            s.step(1)
+            tr.append(s.get_fields()[0][0][0, 0, 4])
+        tr = np.array(tr); t = (np.arange(300) + 1) * dt
+        sg = np.sign(tr); idx = np.where(sg[:-1] * sg[1:] < 0)[0]
+        tz = t[idx] - tr[idx] * (t[idx + 1] - t[idx]) / (tr[idx + 1] - tr[idx])
+        freqs.append(math.pi * (len(tz) - 1) / (tz[-1] - tz[0]))
+    assert abs(freqs[0] - freqs[1]) < 1e-3 * freqs[0]
+    wp = math.sqrt(1e24 * W.Q_E ** 2 / (W.EPS0 * W.M_E))
+    assert 0.96 < freqs[1] / wp < 1.001
+
+
+def test_pool_makes_no_allocations_in_steady_state():
+    """no cudaMalloc/cudaFree during time steps."""
+    cfg = small("C2", (16, 16, 16))
+    _, g, _ = make_pair(cfg, with_oracle=False)
+    g.step(5)
+    d0 = g.diagnostics()
+    g.step(12)
+    g.get_fields(); g.get_particles()
+    d1 = g.diagnostics()
+    assert d1["pool_chunks"] == d0["pool_chunks"] and d1["pool_bytes"] == d0["pool_bytes"]
+    assert d1["launches"] > d0["launches"]
