@@ -20,8 +20,18 @@ template <class R> void launch_unpack(const Grid<R>& g, const R* padded_src, R* 
 // ---- particles.cu
 enum { kDepositGlobal = 1, kDepositCoop = 2 };
 template <class R>
-void launch_particles(const Grid<R>& g, const Particles<R>& p, int order, int mode,
-                      unsigned long long* deactivated, Ctx& c);
+struct ParticleStep {
+  Particles<R> cur;                  // x^n, u^{n-1/2}, w
+  Particles<R> alt;                  // the other buffer set: its x,y,z receive x^{n+1} (COOP)
+  const int32_t* cell_sorted;        // cell of every slot at the last sort, or nullptr
+  int32_t* stray_list;               // scratch: indices left to kernel 3 (capacity n)
+  unsigned int* stray_count;
+  unsigned long long* deactivated;
+};
+// One particle step of a species. Returns true if the new positions are in alt.{x,y,z}
+// (the caller swaps the position pointers of the two buffer sets), false if updated in place.
+template <class R>
+bool launch_particles(const Grid<R>& g, const ParticleStep<R>& a, int order, int mode, Ctx& c);
 
 // ---- sort.cu
 struct SortScratch {
@@ -32,6 +42,8 @@ struct SortScratch {
   int64_t cap = 0;                // particles the buffers are sized for
   int64_t hist_len = 0;
   int64_t scan_len = 0;
+  int32_t* stray_list = nullptr;  // particles.cu: indices handed to the per-particle kernel
+  unsigned int* stray_count = nullptr;
 };
 int64_t sort_chunk();                                  // keys per block of a radix pass
 int64_t sort_hist_len(int64_t n);                      // entries of `hist` for n particles

@@ -1,173 +1,21 @@
-// Fused field gather + relativistic Boris push + Esirkepov current deposition + wrap
-// (steps 2a-2g; PAPER.md:114 fused gather+push with no per-particle
-// E/B stored; PAPER.md:167-175 deposition; ref [8] Esirkepov PAPER.md:301).
+// Particle kernels: fused field gather + relativistic Boris push, and
+// Esirkepov current deposition in two designs that compute the same sums:
+//   GLOBAL  one thread per particle, gather+push+deposit fused, one global reduction per
+//           particle-node (the paper's GPU design);
+//   COOP    gather+push kernel (one thread per particle), then a warp-cooperative deposition:
+//           a warp walks its cell-sorted particles, lanes own the (j,k) nodes of the cell's
+//           window, x runs along registers; sums stay in registers for a whole run of cells
+//           along x and reach memory once per node (fp64/fp32 reductions at L2).
+// PAPER.md:114 (fused gather+push, no per-particle E/B), PAPER.md:167-175 (deposition),
+// ref [8] Esirkepov PAPER.md:301.
+#include <climits>
+
 #include "internal.h"
+#include "particle_math.cuh"
 
 namespace pic {
 
 namespace {
-
-// ------------------------------------------------------------------ gather
-// Tensor-product interpolation of one component, nested so each inner sum is reused:
-// (n+1)^3 + (n+1)^2 + (n+1) FMAs.
-template <class R, int ORDER>
-__device__ __forceinline__ R interp(const R* __restrict__ F, int base, int sy, int sz,
-                                    const R* wx, const R* wy, const R* wz) {
-  R acc = 0;
-#pragma unroll
-  for (int c = 0; c <= ORDER; ++c) {
-    R accb = 0;
-#pragma unroll
-    for (int b = 0; b <= ORDER; ++b) {
-      R acca = 0;
-#pragma unroll
-      for (int a = 0; a <= ORDER; ++a) acca += wx[a] * __ldg(F + base + a + sy * b + sz * c);
-      accb += wy[b] * acca;
-    }
-    acc += wz[c] * accb;
-  }
-  return acc;
-}
-
-template <class R, int ORDER>
-__device__ __forceinline__ void gather6(const Grid<R>& g, R x, R y, R z, R* E, R* B) {
-  // nodal (offset 0) and staggered (offset 1/2) weight sets per axis, shared by the components
-  R wn[3][ORDER + 1], ws[3][ORDER + 1];
-  int ln[3], ls[3];
-  R pos[3] = {x, y, z};
-#pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    R xi = pos[d] * g.inv_dx[d];
-    ln[d] = shape<R, ORDER>(xi, wn[d]);
-    ls[d] = shape<R, ORDER>(xi - R(0.5), ws[d]);
-    // memory safety if a position ever went non-finite: keep the stencil inside the padded box
-    ln[d] = min(max(ln[d], -kGuard), g.N[d] + kGuard - ORDER - 1);
-    ls[d] = min(max(ls[d], -kGuard), g.N[d] + kGuard - ORDER - 1);
-  }
-  const int sy = g.sy, sz = g.sz;
-  // Ex (s,n,n)  Ey (n,s,n)  Ez (n,n,s)  Bx (n,s,s)  By (s,n,s)  Bz (s,s,n)
-  E[0] = interp<R, ORDER>(g.F[0], g.idx(ls[0], ln[1], ln[2]), sy, sz, ws[0], wn[1], wn[2]);
-  E[1] = interp<R, ORDER>(g.F[1], g.idx(ln[0], ls[1], ln[2]), sy, sz, wn[0], ws[1], wn[2]);
-  E[2] = interp<R, ORDER>(g.F[2], g.idx(ln[0], ln[1], ls[2]), sy, sz, wn[0], wn[1], ws[2]);
-  B[0] = interp<R, ORDER>(g.F[3], g.idx(ln[0], ls[1], ls[2]), sy, sz, wn[0], ws[1], ws[2]);
-  B[1] = interp<R, ORDER>(g.F[4], g.idx(ls[0], ln[1], ls[2]), sy, sz, ws[0], wn[1], ws[2]);
-  B[2] = interp<R, ORDER>(g.F[5], g.idx(ls[0], ls[1], ln[2]), sy, sz, ws[0], ws[1], wn[2]);
-}
-
-// ------------------------------------------------------------------ Boris
-template <class R>
-__device__ __forceinline__ void boris(R kq, R inv_c2, const R* E, const R* B, R* u) {
-  R um0 = u[0] + kq * E[0], um1 = u[1] + kq * E[1], um2 = u[2] + kq * E[2];
-  R ig = R(1) / sqrt(R(1) + (um0 * um0 + um1 * um1 + um2 * um2) * inv_c2);
-  R t0 = kq * B[0] * ig, t1 = kq * B[1] * ig, t2 = kq * B[2] * ig;
-  R up0 = um0 + (um1 * t2 - um2 * t1);
-  R up1 = um1 + (um2 * t0 - um0 * t2);
-  R up2 = um2 + (um0 * t1 - um1 * t0);
-  R sc = R(2) / (R(1) + (t0 * t0 + t1 * t1 + t2 * t2));
-  R s0 = t0 * sc, s1 = t1 * sc, s2 = t2 * sc;
-  u[0] = um0 + (up1 * s2 - up2 * s1) + kq * E[0];
-  u[1] = um1 + (up2 * s0 - up0 * s2) + kq * E[1];
-  u[2] = um2 + (up0 * s1 - up1 * s0) + kq * E[2];
-}
-
-// ------------------------------------------------------------------ Esirkepov, per axis set-up
-// Old and new nodal weights on a COMPACT window of ORDER+2 nodes that starts at grid index
-// `base` = min(l0, l1): the (ORDER+3)-wide window of the definition minus the slot that holds
-// neither (identical sums; reading Q5).
-template <class R, int ORDER>
-__device__ __forceinline__ int esirkepov_axis(R xi0, R xi1, R* S0, R* DS) {
-  constexpr int NW = ORDER + 2;
-  R w0[ORDER + 1], w1[ORDER + 1];
-  int l0 = shape<R, ORDER>(xi0, w0);
-  int l1 = shape<R, ORDER>(xi1, w1);
-  int sh = l1 - l0;                 // -1, 0, +1 (CFL)
-  bool o0 = sh < 0;                 // old weights start at slot 1 when the particle moved down
-  bool o1 = sh > 0;                 // new weights start at slot 1 when it moved up
-#pragma unroll
-  for (int i = 0; i < NW; ++i) {
-    R a_lo = i <= ORDER ? w0[i <= ORDER ? i : 0] : R(0);
-    R a_hi = i >= 1 ? w0[i >= 1 ? i - 1 : 0] : R(0);
-    R b_lo = i <= ORDER ? w1[i <= ORDER ? i : 0] : R(0);
-    R b_hi = i >= 1 ? w1[i >= 1 ? i - 1 : 0] : R(0);
-    S0[i] = o0 ? a_hi : a_lo;
-    DS[i] = (o1 ? b_hi : b_lo) - S0[i];
-  }
-  return o0 ? l1 : l0;
-}
-
-// One thread per particle, one global reduction per particle-node.
-template <class R, int ORDER>
-__device__ __forceinline__ void deposit_global(const Grid<R>& g, const R* jf, R wq, const R* x0, const R* x1) {
-  constexpr int NW = ORDER + 2;
-  R S0[3][NW], DS[3][NW];
-  int b[3];
-#pragma unroll
-  for (int d = 0; d < 3; ++d) {
-    b[d] = esirkepov_axis<R, ORDER>(x0[d] * g.inv_dx[d], x1[d] * g.inv_dx[d], S0[d], DS[d]);
-    b[d] = min(max(b[d], -kGuard), g.N[d] + kGuard - NW);
-  }
-  const int base = g.idx(b[0], b[1], b[2]);
-  const int sy = g.sy, sz = g.sz;
-  const R half = R(0.5), third = R(1) / R(3);
-  const R fx = -(wq * jf[0]), fy = -(wq * jf[1]), fz = -(wq * jf[2]);
-  R* __restrict__ Jx = g.J[0];
-  R* __restrict__ Jy = g.J[1];
-  R* __restrict__ Jz = g.J[2];
-#pragma unroll
-  for (int k = 0; k < NW; ++k)
-#pragma unroll
-    for (int j = 0; j < NW; ++j) {
-      R c = S0[1][j] * S0[2][k] + half * DS[1][j] * S0[2][k] + half * S0[1][j] * DS[2][k] + third * DS[1][j] * DS[2][k];
-      R pre = 0;
-#pragma unroll
-      for (int i = 0; i < NW - 1; ++i) {
-        pre += DS[0][i] * c;
-        R v = fx * pre;
-        if (v != R(0)) red_add(Jx + base + i + sy * j + sz * k, v);
-      }
-    }
-#pragma unroll
-  for (int k = 0; k < NW; ++k)
-#pragma unroll
-    for (int i = 0; i < NW; ++i) {
-      R c = S0[0][i] * S0[2][k] + half * DS[0][i] * S0[2][k] + half * S0[0][i] * DS[2][k] + third * DS[0][i] * DS[2][k];
-      R pre = 0;
-#pragma unroll
-      for (int j = 0; j < NW - 1; ++j) {
-        pre += DS[1][j] * c;
-        R v = fy * pre;
-        if (v != R(0)) red_add(Jy + base + i + sy * j + sz * k, v);
-      }
-    }
-#pragma unroll
-  for (int j = 0; j < NW; ++j)
-#pragma unroll
-    for (int i = 0; i < NW; ++i) {
-      R c = S0[0][i] * S0[1][j] + half * DS[0][i] * S0[1][j] + half * S0[0][i] * DS[1][j] + third * DS[0][i] * DS[1][j];
-      R pre = 0;
-#pragma unroll
-      for (int k = 0; k < NW - 1; ++k) {
-        pre += DS[2][k] * c;
-        R v = fz * pre;
-        if (v != R(0)) red_add(Jz + base + i + sy * j + sz * k, v);
-      }
-    }
-}
-
-// periodic wrap / deactivation, exactly the sequence of DESIGN.md step 2f
-template <class R>
-__device__ __forceinline__ bool wrap_axis(R& x, R L, int periodic) {
-  if (periodic) {
-    if (x < R(0)) x += L;
-    if (x >= L) x -= L;
-    return false;
-  }
-  if (!(x >= R(0) && x < L)) {
-    x = x < R(0) ? R(0) : nextafter(L, R(0));
-    return true;
-  }
-  return false;
-}
 
 template <class R, int ORDER>
 __global__ void __launch_bounds__(128) k_particles_global(Grid<R> g, Particles<R> p, unsigned long long* deactivated) {
@@ -193,28 +41,284 @@ __global__ void __launch_bounds__(128) k_particles_global(Grid<R> g, Particles<R
   p.ux[t] = u[0]; p.uy[t] = u[1]; p.uz[t] = u[2];
 }
 
+// ------------------------------------------------------------------ COOP, kernel 1: gather + push
+// Reads x^n, u^{n-1/2}; writes u^{n+1/2} in place and the UNWRAPPED new position into `xn`.
 template <class R, int ORDER>
-void launch_global(const Grid<R>& g, const Particles<R>& p, unsigned long long* deact, Ctx& c) {
-  if (p.n == 0) return;
-  int64_t nb = (p.n + 127) / 128;
-  k_particles_global<R, ORDER><<<(unsigned)nb, 128, 0, c.stream>>>(g, p, deact);
-  c.launches++;
+__global__ void __launch_bounds__(128) k_push(Grid<R> g, Particles<R> p, R* __restrict__ xn, R* __restrict__ yn,
+                                              R* __restrict__ zn) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= p.n) return;
+  R x0[3] = {p.x[t], p.y[t], p.z[t]};
+  R u[3] = {p.ux[t], p.uy[t], p.uz[t]};
+  R E[3], B[3];
+  gather6<R, ORDER>(g, x0[0], x0[1], x0[2], E, B);
+  boris<R>(p.kq, g.inv_c2, E, B, u);
+  R ig = g.dt / sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * g.inv_c2);
+  xn[t] = x0[0] + u[0] * ig;
+  yn[t] = x0[1] + u[1] * ig;
+  zn[t] = x0[2] + u[2] * ig;
+  p.ux[t] = u[0]; p.uy[t] = u[1]; p.uz[t] = u[2];
+}
+
+// ------------------------------------------------------------------ COOP, kernel 2: deposition
+template <class R>
+struct alignas(2 * sizeof(R)) Pair { R a, b; };
+
+template <int ORDER>
+struct Win {
+  static constexpr int NW = ORDER == 1 ? 4 : 6;   // nodes per axis of the window fixed to a CELL
+  static constexpr int BL = ORDER == 1 ? 1 : 2;   // window base = cell - BL
+  static constexpr int REC = 9 * NW + (NW == 4 ? 2 : 0);   // record stride: conflict-free stores
+  // record layout (elements): {A_x,B_x}[NW] | {S0_y,DS_y}[NW] | {S0_z,DS_z}[NW] | PX[NW] | PY[NW] | PZ[NW]
+  static constexpr int oABX = 0, oY = 2 * NW, oZ = 4 * NW, oPX = 6 * NW, oPY = 7 * NW, oPZ = 8 * NW;
+};
+
+constexpr int kCoopWarps = 4;        // warps per CTA
+constexpr int kCoopChunk = 512;      // consecutive particles walked by one warp
+
+// Per axis: old/new weights placed on the cell's window, DS, A = S0 + DS/2, B = S0/2 + DS/3 and
+// the running sum of DS (Esirkepov: W_x = DS_x (S0_z A_y + DS_z B_y), J_x = -q w/(dt dy dz) cumsum_x W_x, cyclic).
+template <class R, int ORDER>
+__device__ __forceinline__ void axis_record(R xi0, R xi1, int N, int& cell, R* S0, R* DS, bool& edge) {
+  constexpr int NW = Win<ORDER>::NW, BL = Win<ORDER>::BL;
+  R w0[ORDER + 1], w1[ORDER + 1];
+  int l0 = shape<R, ORDER>(xi0, w0);
+  int l1 = shape<R, ORDER>(xi1, w1);
+  int c = ORDER == 2 ? (int)floor(xi0) : (ORDER == 1 ? l0 : l0 + 1);
+  c = min(max(c, 0), N);
+  int so0 = l0 - (c - BL), sl1 = l1 - (c - BL);
+  R S1[NW];
+#pragma unroll
+  for (int i = 0; i < NW; ++i) {
+    R a = 0, b = 0;
+#pragma unroll
+    for (int k = 0; k <= ORDER; ++k) {
+      a = (i == so0 + k) ? w0[k] : a;
+      b = (i == sl1 + k) ? w1[k] : b;
+    }
+    S0[i] = a;
+    S1[i] = b;
+    DS[i] = b - a;
+  }
+  edge = (S0[0] != R(0)) | (S1[0] != R(0)) | (S0[NW - 1] != R(0)) | (S1[NW - 1] != R(0));
+  cell = c;
+}
+
+template <class R, int ORDER>
+__global__ void __launch_bounds__(kCoopWarps * 32) k_deposit_coop(Grid<R> g, Particles<R> p, R* __restrict__ xn,
+                                                                  R* __restrict__ yn, R* __restrict__ zn,
+                                                                  const int32_t* __restrict__ cell_sorted,
+                                                                  int32_t* __restrict__ stray_list,
+                                                                  unsigned int* __restrict__ stray_count,
+                                                                  unsigned long long* deactivated) {
+  using W = Win<ORDER>;
+  constexpr int NW = W::NW, BL = W::BL, REC = W::REC;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  R* rec = reinterpret_cast<R*>(smem_raw) + (size_t)warp * 32 * REC;
+  // lane -> (j,k) of the window; the 6x6 window has 36 pairs: its 4 corners are never needed by
+  // the particles this kernel accepts (a corner needs a cell change in y AND z; those go to the list)
+  int pair = lane;
+  bool lane_on = true;
+  if (NW == 6) pair = lane < 4 ? lane + 1 : (lane < 28 ? lane + 2 : lane + 3);
+  else lane_on = lane < NW * NW;
+  const int j = lane_on ? pair / NW : 0, k = lane_on ? pair % NW : 0;
+  const int off_jk = g.sy * j + g.sz * k;
+  const R half = R(0.5), third = R(1) / R(3);
+
+  R ax[NW - 1], ay[NW], az[NW];
+#pragma unroll
+  for (int i = 0; i < NW; ++i) { ay[i] = 0; az[i] = 0; if (i < NW - 1) ax[i] = 0; }
+  int cur_ib = INT_MIN;    // window base index of the run being accumulated
+
+  auto flush_all = [&]() {
+    if (cur_ib == INT_MIN || !lane_on) return;
+    R* jx = g.J[0] + cur_ib + off_jk;
+    R* jy = g.J[1] + cur_ib + off_jk;
+    R* jz = g.J[2] + cur_ib + off_jk;
+#pragma unroll
+    for (int i = 0; i < NW; ++i) {
+      if (i < NW - 1 && ax[i] != R(0)) red_add(jx + i, ax[i]);
+      if (ay[i] != R(0)) red_add(jy + i, ay[i]);
+      if (az[i] != R(0)) red_add(jz + i, az[i]);
+    }
+  };
+  auto zero_all = [&]() {
+#pragma unroll
+    for (int i = 0; i < NW; ++i) { ay[i] = 0; az[i] = 0; if (i < NW - 1) ax[i] = 0; }
+  };
+  auto shift_one = [&]() {   // the run moves one cell up in x: x-slot 0 is complete
+    if (lane_on) {
+      if (ax[0] != R(0)) red_add(g.J[0] + cur_ib + off_jk, ax[0]);
+      if (ay[0] != R(0)) red_add(g.J[1] + cur_ib + off_jk, ay[0]);
+      if (az[0] != R(0)) red_add(g.J[2] + cur_ib + off_jk, az[0]);
+    }
+#pragma unroll
+    for (int i = 0; i < NW - 1; ++i) { ay[i] = ay[i + 1]; az[i] = az[i + 1]; if (i < NW - 2) ax[i] = ax[i + 1]; }
+    ay[NW - 1] = 0; az[NW - 1] = 0; ax[NW - 2] = 0;
+    cur_ib += 1;
+  };
+
+  const int64_t wg = (int64_t)blockIdx.x * kCoopWarps + warp;
+  const int64_t begin = wg * kCoopChunk;
+  const int64_t end = min(p.n, begin + kCoopChunk);
+  for (int64_t b0 = begin; b0 < end; b0 += 32) {
+    const int64_t t = b0 + lane;
+    const bool valid = t < end;
+    bool elig = false;
+    int ib = 0;
+    R x1[3] = {0, 0, 0};
+    R w = 0;
+    if (valid) {
+      R x0[3] = {p.x[t], p.y[t], p.z[t]};
+      x1[0] = xn[t]; x1[1] = yn[t]; x1[2] = zn[t];
+      w = p.w[t];
+      R S0[3][NW], DS[3][NW];
+      int c[3];
+      bool edge[3];
+#pragma unroll
+      for (int d = 0; d < 3; ++d)
+        axis_record<R, ORDER>(x0[d] * g.inv_dx[d], x1[d] * g.inv_dx[d], g.N[d], c[d], S0[d], DS[d], edge[d]);
+      elig = cell_sorted == nullptr || cell_sorted[t] == c[0] + g.N[0] * (c[1] + g.N[1] * c[2]);
+      if (NW * NW > 32) elig &= !(edge[1] && edge[2]);
+      if (elig) {
+        ib = g.idx(c[0] - BL, c[1] - BL, c[2] - BL);
+        R* r = rec + lane * REC;
+        const R fx = -(w * p.jf[0]), fy = -(w * p.jf[1]), fz = -(w * p.jf[2]);
+        R px = 0, py = 0, pz = 0;
+#pragma unroll
+        for (int i = 0; i < NW; ++i) {
+          Pair<R> ab{S0[0][i] + half * DS[0][i], half * S0[0][i] + third * DS[0][i]};
+          *reinterpret_cast<Pair<R>*>(r + W::oABX + 2 * i) = ab;
+          *reinterpret_cast<Pair<R>*>(r + W::oY + 2 * i) = Pair<R>{S0[1][i], DS[1][i]};
+          *reinterpret_cast<Pair<R>*>(r + W::oZ + 2 * i) = Pair<R>{S0[2][i], DS[2][i]};
+          px += DS[0][i]; py += DS[1][i]; pz += DS[2][i];
+          r[W::oPX + i] = fx * px;
+          r[W::oPY + i] = fy * py;
+          r[W::oPZ + i] = fz * pz;
+        }
+      }
+    }
+    __syncwarp();
+    unsigned m = __ballot_sync(0xffffffffu, elig);
+    while (m) {
+      const int q = __ffs(m) - 1;
+      m &= m - 1;
+      const int ibq = __shfl_sync(0xffffffffu, ib, q);
+      if (ibq != cur_ib) {
+        const int s = ibq - cur_ib;
+        if (cur_ib != INT_MIN && s > 0 && s < NW) {
+          for (int e = 0; e < s; ++e) shift_one();
+        } else {
+          flush_all();
+          zero_all();
+          cur_ib = ibq;
+        }
+      }
+      const R* r = rec + q * REC;
+      const Pair<R> yv = *reinterpret_cast<const Pair<R>*>(r + W::oY + 2 * j);
+      const Pair<R> zv = *reinterpret_cast<const Pair<R>*>(r + W::oZ + 2 * k);
+      const R py = r[W::oPY + j], pz = r[W::oPZ + k];
+      const R cx = zv.a * (yv.a + half * yv.b) + zv.b * (half * yv.a + third * yv.b);
+      const R q1 = py * zv.a, q2 = py * zv.b;
+      const R r1 = pz * yv.a, r2 = pz * yv.b;
+#pragma unroll
+      for (int i = 0; i < NW; ++i) {
+        const Pair<R> ab = *reinterpret_cast<const Pair<R>*>(r + W::oABX + 2 * i);
+        if (i < NW - 1) ax[i] += cx * r[W::oPX + i];
+        ay[i] += q1 * ab.a + q2 * ab.b;
+        az[i] += r1 * ab.a + r2 * ab.b;
+      }
+    }
+    __syncwarp();
+    // particles deposited here are finished: wrap and store; the others go to the list untouched
+    const bool stray = valid && !elig;
+    const unsigned sm = __ballot_sync(0xffffffffu, stray);
+    if (sm) {
+      unsigned base = 0;
+      if (lane == 0) base = atomicAdd(stray_count, (unsigned)__popc(sm));
+      base = __shfl_sync(0xffffffffu, base, 0);
+      if (stray) stray_list[base + __popc(sm & ((1u << lane) - 1u))] = (int32_t)t;
+    }
+    if (valid && elig) {
+      bool out = false;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) out |= wrap_axis<R>(x1[d], g.L[d], g.periodic[d]);
+      if (out) {
+        if (w != R(0)) atomicAdd(deactivated, 1ull);
+        p.w[t] = R(0);
+      }
+      xn[t] = x1[0]; yn[t] = x1[1]; zn[t] = x1[2];
+    }
+  }
+  flush_all();
+}
+
+// ------------------------------------------------------------------ COOP, kernel 3: the listed particles
+// (changed cell since the last sort, or changed cell in y and z at once): one thread each, global
+// reductions, as in the GLOBAL design.
+template <class R, int ORDER>
+__global__ void __launch_bounds__(128) k_deposit_list(Grid<R> g, Particles<R> p, R* __restrict__ xn, R* __restrict__ yn,
+                                                      R* __restrict__ zn, const int32_t* __restrict__ list,
+                                                      const unsigned int* __restrict__ count,
+                                                      unsigned long long* deactivated) {
+  const unsigned n = *count;
+  for (unsigned e = blockIdx.x * blockDim.x + threadIdx.x; e < n; e += gridDim.x * blockDim.x) {
+    const int t = list[e];
+    R x0[3] = {p.x[t], p.y[t], p.z[t]};
+    R x1[3] = {xn[t], yn[t], zn[t]};
+    R w = p.w[t];
+    deposit_global<R, ORDER>(g, p.jf, w, x0, x1);
+    bool out = false;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) out |= wrap_axis<R>(x1[d], g.L[d], g.periodic[d]);
+    if (out) {
+      if (w != R(0)) atomicAdd(deactivated, 1ull);
+      p.w[t] = R(0);
+    }
+    xn[t] = x1[0]; yn[t] = x1[1]; zn[t] = x1[2];
+  }
+}
+
+template <class R, int ORDER>
+bool launch_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) {
+  const Particles<R>& p = a.cur;
+  if (p.n == 0) return false;
+  if (mode != kDepositCoop) {
+    int64_t nb = (p.n + 127) / 128;
+    k_particles_global<R, ORDER><<<(unsigned)nb, 128, 0, c.stream>>>(g, p, a.deactivated);
+    c.launches++;
+    return false;
+  }
+  R *xn = a.alt.x, *yn = a.alt.y, *zn = a.alt.z;
+  k_push<R, ORDER><<<(unsigned)((p.n + 127) / 128), 128, 0, c.stream>>>(g, p, xn, yn, zn);
+  cudaMemsetAsync(a.stray_count, 0, sizeof(unsigned int), c.stream);
+  const size_t smem = (size_t)kCoopWarps * 32 * Win<ORDER>::REC * sizeof(R);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(k_deposit_coop<R, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attr_set = true;
+  }
+  const int64_t per_cta = (int64_t)kCoopWarps * kCoopChunk;
+  k_deposit_coop<R, ORDER><<<(unsigned)((p.n + per_cta - 1) / per_cta), kCoopWarps * 32, smem, c.stream>>>(
+      g, p, xn, yn, zn, a.cell_sorted, a.stray_list, a.stray_count, a.deactivated);
+  k_deposit_list<R, ORDER><<<148 * 4, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count, a.deactivated);
+  c.launches += 3;
+  return true;
 }
 
 }  // namespace
 
 template <class R>
-void launch_particles(const Grid<R>& g, const Particles<R>& p, int order, int mode,
-                      unsigned long long* deactivated, Ctx& c) {
-  (void)mode;
+bool launch_particles(const Grid<R>& g, const ParticleStep<R>& a, int order, int mode, Ctx& c) {
   switch (order) {
-    case 1: launch_global<R, 1>(g, p, deactivated, c); break;
-    case 2: launch_global<R, 2>(g, p, deactivated, c); break;
-    default: launch_global<R, 3>(g, p, deactivated, c); break;
+    case 1: return launch_order<R, 1>(g, a, mode, c);
+    case 2: return launch_order<R, 2>(g, a, mode, c);
+    default: return launch_order<R, 3>(g, a, mode, c);
   }
 }
 
-template void launch_particles<double>(const Grid<double>&, const Particles<double>&, int, int, unsigned long long*, Ctx&);
-template void launch_particles<float>(const Grid<float>&, const Particles<float>&, int, int, unsigned long long*, Ctx&);
+template bool launch_particles<double>(const Grid<double>&, const ParticleStep<double>&, int, int, Ctx&);
+template bool launch_particles<float>(const Grid<float>&, const ParticleStep<float>&, int, int, Ctx&);
 
 }  // namespace pic

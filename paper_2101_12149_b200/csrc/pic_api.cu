@@ -7,6 +7,7 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "internal.h"
@@ -192,6 +193,8 @@ struct Sim : SimBase {
     for (int i = 0; i < 2; ++i) { pool.free(scratch.keys[i]); pool.free(scratch.vals[i]); }
     pool.free(scratch.hist);
     pool.free(scratch.scan_tmp);
+    pool.free(scratch.stray_list);
+    pool.free(scratch.stray_count);
     scratch = SortScratch();
     scratch.hist_len = sort_hist_len(n);
     scratch.scan_len = sort_scan_tmp_len(scratch.hist_len);
@@ -202,7 +205,10 @@ struct Sim : SimBase {
     }
     scratch.hist = palloc<uint32_t>((size_t)scratch.hist_len);
     scratch.scan_tmp = palloc<uint32_t>((size_t)scratch.scan_len);
-    if (!scratch.hist || !scratch.scan_tmp) return fail(PIC_ERR_OOM, "sort scratch allocation failed");
+    scratch.stray_list = palloc<int32_t>((size_t)n);
+    scratch.stray_count = palloc<unsigned int>(1);
+    if (!scratch.hist || !scratch.scan_tmp || !scratch.stray_list || !scratch.stray_count)
+      return fail(PIC_ERR_OOM, "sort scratch allocation failed");
     scratch.cap = n;
     return PIC_OK;
   }
@@ -340,6 +346,27 @@ struct Sim : SimBase {
     }
   }
 
+  // AUTO: the warp-cooperative deposition needs the cell-sorted order to pay off
+  int pick_mode(const Species<R>& sp) const {
+    if (deposit_mode != PIC_DEPOSIT_AUTO) return deposit_mode;
+    return sp.sorted_once ? kDepositCoop : kDepositGlobal;
+  }
+  void particle_step(Species<R>& sp) {
+    ParticleStep<R> a;
+    a.cur = sp.buf[sp.cur];
+    a.alt = sp.buf[sp.cur ^ 1];
+    a.cell_sorted = sp.sorted_once ? sp.cell : nullptr;
+    a.stray_list = scratch.stray_list;
+    a.stray_count = scratch.stray_count;
+    a.deactivated = d_deact;
+    if (launch_particles<R>(g, a, order, pick_mode(sp), ctx)) {
+      Particles<R>&c0 = sp.buf[sp.cur], &c1 = sp.buf[sp.cur ^ 1];
+      std::swap(c0.x, c1.x);
+      std::swap(c0.y, c1.y);
+      std::swap(c0.z, c1.z);
+    }
+  }
+
   int step(int n) override {
     if (n < 0) return fail(PIC_ERR_INVALID_ARG, "negative step count");
     const size_t jbytes = (size_t)g.padded_total() * 3 * sizeof(R);
@@ -359,7 +386,7 @@ struct Sim : SimBase {
       {
         Phase ph(this, PIC_PHASE_PARTICLES);
         cudaMemsetAsync(g.J[0], 0, jbytes, ctx.stream);   // the three J arrays are contiguous
-        for (auto& sp : species) launch_particles<R>(g, sp.buf[sp.cur], order, deposit_mode, d_deact, ctx);
+        for (auto& sp : species) particle_step(sp);
       }
       {
         Phase ph(this, PIC_PHASE_FIELDS);
