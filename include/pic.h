@@ -147,19 +147,31 @@ enum {
   PIC_DIAG_STEPS = 7,       /* steps taken */
   PIC_DIAG_POOL_CHUNKS = 8, /* cudaMalloc calls made by the memory pool so far */
   PIC_DIAG_POOL_BYTES = 9,  /* bytes held by the pool */
-  PIC_DIAG_LAUNCHES = 10,   /* kernels launched by this handle so far */
-  PIC_NDIAG = 11
+  PIC_DIAG_LAUNCHES = 10,   /* kernels launched by this handle so far (all calls) */
+  PIC_DIAG_STEP_LAUNCHES = 11, /* kernels launched by pic_step and pic_sort_now so far */
+  PIC_NDIAG = 12
 };
 PIC_API int pic_get_diagnostics(pic_sim* sim, double* out);
 
 /* Nodal charge density rho (C/m^3, fp64, n_x*n_y*n_z, x fastest) of all species. Synchronises. */
 PIC_API int pic_get_rho(pic_sim* sim, double* rho, pic_mem where);
 
-/* Elapsed device time (ms) spent in each phase since the last call with reset != 0; host array
- * of PIC_NPHASE floats. Phase timing is off until pic_enable_phase_timing(sim, 1). */
-enum { PIC_PHASE_SORT = 0, PIC_PHASE_PARTICLES = 1, PIC_PHASE_FIELDS = 2, PIC_NPHASE = 3 };
+/* Device time per kernel class, from CUDA events recorded on the simulation's stream around each
+ * launch group (never synchronises while stepping). ms[p] = elapsed time (ms) summed over the
+ * spans of class p since the last call with reset != 0, spans[p] (nullable) = how many spans that
+ * was (one span = one launch of that class's kernel for PUSH / DEPOSIT / STRAY, one whole sort
+ * for SORT, one launch group for FIELDS). Host arrays of PIC_NPHASE elements. Timing is off
+ * until pic_enable_phase_timing(sim, 1). pic_get_phase_times synchronises. */
+enum {
+  PIC_PHASE_SORT = 0,    /* keys, radix passes, permutation of all attributes */
+  PIC_PHASE_PUSH = 1,    /* gather + Boris push (+ deposit when PIC_DEPOSIT_GLOBAL fuses it) */
+  PIC_PHASE_DEPOSIT = 2, /* warp-cooperative Esirkepov deposition */
+  PIC_PHASE_STRAY = 3,   /* per-particle deposition of the particles the cooperative kernel skipped */
+  PIC_PHASE_FIELDS = 4,  /* J zero, J guard sum, Yee B/E/B, guard fill */
+  PIC_NPHASE = 5
+};
 PIC_API int pic_enable_phase_timing(pic_sim* sim, int32_t on);
-PIC_API int pic_get_phase_times(pic_sim* sim, float* ms, int32_t reset);
+PIC_API int pic_get_phase_times(pic_sim* sim, float* ms, int64_t* spans, int32_t reset);
 
 PIC_API int64_t pic_num_particles(const pic_sim* sim, int32_t species); /* < 0 on error */
 PIC_API int32_t pic_num_species(const pic_sim* sim);

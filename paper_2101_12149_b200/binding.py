@@ -15,11 +15,11 @@ LIB_PATH = os.path.join(_HERE, "libpic.so")
 PIC_F64, PIC_F32 = 0, 1
 PIC_HOST, PIC_DEVICE = 0, 1
 PIC_DEPOSIT_AUTO, PIC_DEPOSIT_GLOBAL, PIC_DEPOSIT_COOP = 0, 1, 2
-PIC_NDIAG = 11
-PIC_NPHASE = 3
+PIC_NDIAG = 12
+PIC_NPHASE = 5
 DIAG_NAMES = ("field_E", "field_B", "kinetic", "charge", "gauss_max", "rho_max", "deactivated", "steps",
-              "pool_chunks", "pool_bytes", "launches")
-PHASE_NAMES = ("sort", "particles", "fields")
+              "pool_chunks", "pool_bytes", "launches", "step_launches")
+PHASE_NAMES = ("sort", "push", "deposit", "stray", "fields")
 ERRORS = {-1: "PIC_ERR_INVALID_ARG", -2: "PIC_ERR_CFL", -3: "PIC_ERR_OUT_OF_DOMAIN", -4: "PIC_ERR_OOM",
           -5: "PIC_ERR_CUDA", -6: "PIC_ERR_CAPACITY"}
 
@@ -71,7 +71,7 @@ def lib():
         L.pic_get_diagnostics.argtypes = [vp, dp]
         L.pic_get_rho.argtypes = [vp, vp, C.c_int]
         L.pic_enable_phase_timing.argtypes = [vp, C.c_int32]
-        L.pic_get_phase_times.argtypes = [vp, C.POINTER(C.c_float), C.c_int32]
+        L.pic_get_phase_times.argtypes = [vp, C.POINTER(C.c_float), i64p, C.c_int32]
         L.pic_num_particles.argtypes = [vp, C.c_int32]
         L.pic_num_particles.restype = C.c_int64
         L.pic_num_species.argtypes = [vp]
@@ -201,9 +201,11 @@ def pic_enable_phase_timing(h, on=True):
 
 
 def pic_get_phase_times(h, reset=True) -> dict:
+    """{class: (elapsed ms, spans)} since the last reset."""
     ms = (C.c_float * PIC_NPHASE)()
-    _check(h, lib().pic_get_phase_times(h, ms, 1 if reset else 0))
-    return dict(zip(PHASE_NAMES, ms))
+    cnt = (C.c_int64 * PIC_NPHASE)()
+    _check(h, lib().pic_get_phase_times(h, ms, cnt, 1 if reset else 0))
+    return {k: (float(m), int(c)) for k, m, c in zip(PHASE_NAMES, ms, cnt)}
 
 
 def pic_num_particles(h, species=0) -> int:

@@ -1,13 +1,78 @@
 // Host-side declarations shared by the translation units of libpic.so (CUDA path only).
 #pragma once
+#include <vector>
+
 #include "common.cuh"
 
 namespace pic {
 
+// Per-kernel-class device timers (pic_get_phase_times): CUDA events recorded on the simulation's
+// stream around each launch group. Off unless enabled; recording never synchronises.
+constexpr int kNumPhases = 5;   // == PIC_NPHASE: sort, push, deposit, stray, fields
+struct Timer {
+  struct Span { int phase; cudaEvent_t a, b; };
+  bool on = false;
+  std::vector<Span> spans;
+  std::vector<cudaEvent_t> free_events;
+  float ms[kNumPhases] = {0, 0, 0, 0, 0};
+  int64_t count[kNumPhases] = {0, 0, 0, 0, 0};
+  cudaEvent_t get_event() {
+    if (!free_events.empty()) {
+      cudaEvent_t e = free_events.back();
+      free_events.pop_back();
+      return e;
+    }
+    cudaEvent_t e;
+    cudaEventCreate(&e);
+    return e;
+  }
+  int begin(int phase, cudaStream_t st) {
+    if (!on) return -1;
+    Span sp{phase, get_event(), get_event()};
+    cudaEventRecord(sp.a, st);
+    spans.push_back(sp);
+    return (int)spans.size() - 1;
+  }
+  void end(int idx, cudaStream_t st) {
+    if (idx >= 0) cudaEventRecord(spans[idx].b, st);
+  }
+  void fold() {   // synchronises on the recorded events
+    for (auto& s : spans) {
+      cudaEventSynchronize(s.b);
+      float t = 0;
+      cudaEventElapsedTime(&t, s.a, s.b);
+      ms[s.phase] += t;
+      count[s.phase] += 1;
+      free_events.push_back(s.a);
+      free_events.push_back(s.b);
+    }
+    spans.clear();
+  }
+  void reset() {
+    for (int i = 0; i < kNumPhases; ++i) { ms[i] = 0; count[i] = 0; }
+  }
+  void destroy() {
+    for (auto& s : spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
+    for (auto e : free_events) cudaEventDestroy(e);
+    spans.clear();
+    free_events.clear();
+  }
+};
+
 struct Ctx {
   cudaStream_t stream = nullptr;
   int64_t launches = 0;   // kernels launched through this handle
+  Timer timer;
 };
+
+// times everything launched on c.stream during its lifetime as one span of `phase`
+struct ScopedPhase {
+  Ctx& c;
+  int idx;
+  ScopedPhase(Ctx& c_, int phase) : c(c_), idx(c_.timer.begin(phase, c_.stream)) {}
+  ~ScopedPhase() { c.timer.end(idx, c.stream); }
+};
+enum { kPhaseSort = 0, kPhasePush = 1, kPhaseDeposit = 2, kPhaseStray = 3, kPhaseFields = 4 };
 
 // ---- fields.cu
 template <class R> void launch_push_B(const Grid<R>& g, const int lo[3], const int hi[3], Ctx& c);

@@ -285,13 +285,17 @@ bool launch_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) 
   const Particles<R>& p = a.cur;
   if (p.n == 0) return false;
   if (mode != kDepositCoop) {
+    ScopedPhase ph(c, kPhasePush);
     int64_t nb = (p.n + 127) / 128;
     k_particles_global<R, ORDER><<<(unsigned)nb, 128, 0, c.stream>>>(g, p, a.deactivated);
     c.launches++;
     return false;
   }
   R *xn = a.alt.x, *yn = a.alt.y, *zn = a.alt.z;
-  k_push<R, ORDER><<<(unsigned)((p.n + 127) / 128), 128, 0, c.stream>>>(g, p, xn, yn, zn);
+  {
+    ScopedPhase ph(c, kPhasePush);
+    k_push<R, ORDER><<<(unsigned)((p.n + 127) / 128), 128, 0, c.stream>>>(g, p, xn, yn, zn);
+  }
   cudaMemsetAsync(a.stray_count, 0, sizeof(unsigned int), c.stream);
   const size_t smem = (size_t)kCoopWarps * 32 * Win<ORDER>::REC * sizeof(R);
   static bool attr_set = false;
@@ -300,9 +304,16 @@ bool launch_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) 
     attr_set = true;
   }
   const int64_t per_cta = (int64_t)kCoopWarps * kCoopChunk;
-  k_deposit_coop<R, ORDER><<<(unsigned)((p.n + per_cta - 1) / per_cta), kCoopWarps * 32, smem, c.stream>>>(
-      g, p, xn, yn, zn, a.cell_sorted, a.stray_list, a.stray_count, a.deactivated);
-  k_deposit_list<R, ORDER><<<148 * 4, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count, a.deactivated);
+  {
+    ScopedPhase ph(c, kPhaseDeposit);
+    k_deposit_coop<R, ORDER><<<(unsigned)((p.n + per_cta - 1) / per_cta), kCoopWarps * 32, smem, c.stream>>>(
+        g, p, xn, yn, zn, a.cell_sorted, a.stray_list, a.stray_count, a.deactivated);
+  }
+  {
+    ScopedPhase ph(c, kPhaseStray);
+    k_deposit_list<R, ORDER><<<148 * 4, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count,
+                                                            a.deactivated);
+  }
   c.launches += 3;
   return true;
 }

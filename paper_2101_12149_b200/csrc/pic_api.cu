@@ -15,6 +15,8 @@
 
 namespace pic {
 
+static_assert(kNumPhases == PIC_NPHASE, "phase lists out of sync");
+
 namespace {
 
 thread_local std::string g_create_error;
@@ -39,7 +41,7 @@ struct SimBase {
   virtual int diagnostics(double* out) = 0;
   virtual int get_rho(double* rho, pic_mem where) = 0;
   virtual int enable_timing(int on) = 0;
-  virtual int phase_times(float* ms, int reset) = 0;
+  virtual int phase_times(float* ms, int64_t* launches, int reset) = 0;
   virtual int64_t num_particles(int sp) const = 0;
   virtual int num_species() const = 0;
 };
@@ -67,20 +69,13 @@ struct Sim : SimBase {
   std::vector<Species<R>> species;
   SortScratch scratch;
   int64_t step_count = 0;
+  int64_t step_launches = 0;   // kernels launched by pic_step / pic_sort_now
   unsigned long long* d_deact = nullptr;
   int* d_flags = nullptr;
   double* d_red = nullptr;   // 8 doubles of reduction scratch
-  // phase timing
-  bool timing = false;
-  struct Span { int phase; cudaEvent_t a, b; };
-  std::vector<Span> spans;
-  std::vector<cudaEvent_t> free_events;
-  float phase_ms[PIC_NPHASE] = {0, 0, 0};
-
   ~Sim() override {
     cudaStreamSynchronize(ctx.stream);
-    for (auto& s : spans) { cudaEventDestroy(s.a); cudaEventDestroy(s.b); }
-    for (auto e : free_events) cudaEventDestroy(e);
+    ctx.timer.destroy();
     pool.release();
     cudaGetLastError();
   }
@@ -301,42 +296,6 @@ struct Sim : SimBase {
     return check_launch("set_fields kernels");
   }
 
-  // ---- phase timing
-  cudaEvent_t get_event() {
-    if (!free_events.empty()) {
-      cudaEvent_t e = free_events.back();
-      free_events.pop_back();
-      return e;
-    }
-    cudaEvent_t e;
-    cudaEventCreate(&e);
-    return e;
-  }
-  void fold_spans() {
-    for (auto& s : spans) {
-      cudaEventSynchronize(s.b);
-      float ms = 0;
-      cudaEventElapsedTime(&ms, s.a, s.b);
-      phase_ms[s.phase] += ms;
-      free_events.push_back(s.a);
-      free_events.push_back(s.b);
-    }
-    spans.clear();
-  }
-  struct Phase {
-    Sim* s; int idx = -1;
-    Phase(Sim* s_, int phase) : s(s_) {
-      if (!s->timing) return;
-      Span sp{phase, s->get_event(), s->get_event()};
-      cudaEventRecord(sp.a, s->ctx.stream);
-      s->spans.push_back(sp);
-      idx = (int)s->spans.size() - 1;
-    }
-    ~Phase() {
-      if (idx >= 0) cudaEventRecord(s->spans[idx].b, s->ctx.stream);
-    }
-  };
-
   void do_sort() {
     for (auto& sp : species) {
       if (sp.buf[sp.cur].n == 0) { sp.sorted_once = true; continue; }
@@ -378,18 +337,19 @@ struct Sim : SimBase {
       loE[d] = 0;
       hiE[d] = hiB[d];
     }
+    const int64_t launches0 = ctx.launches;
     for (int s = 0; s < n; ++s) {
       if (sort_interval > 0 && step_count % sort_interval == 0) {
-        Phase ph(this, PIC_PHASE_SORT);
+        ScopedPhase ph(ctx, kPhaseSort);
         do_sort();
       }
       {
-        Phase ph(this, PIC_PHASE_PARTICLES);
+        ScopedPhase ph(ctx, kPhaseFields);
         cudaMemsetAsync(g.J[0], 0, jbytes, ctx.stream);   // the three J arrays are contiguous
-        for (auto& sp : species) particle_step(sp);
       }
+      for (auto& sp : species) particle_step(sp);         // timed per kernel in particles.cu
       {
-        Phase ph(this, PIC_PHASE_FIELDS);
+        ScopedPhase ph(ctx, kPhaseFields);
         launch_fold_J<R>(g, ctx);                    // SumBoundary
         launch_fill_guards<R>(g, g.J, 3, ctx);       // J images for the widened E update
         launch_push_B<R>(g, loB, hiB, ctx);          // widened by one layer on periodic axes, so
@@ -398,8 +358,9 @@ struct Sim : SimBase {
         launch_fill_guards<R>(g, g.F, 6, ctx);       // FillBoundary
       }
       step_count++;
-      if (timing && spans.size() > 3000) fold_spans();
+      if (ctx.timer.spans.size() > 3000) ctx.timer.fold();
     }
+    step_launches += ctx.launches - launches0;
     return check_launch("pic_step launch");
   }
 
@@ -463,8 +424,12 @@ struct Sim : SimBase {
   }
 
   int sort_now() override {
-    Phase ph(this, PIC_PHASE_SORT);
-    do_sort();
+    const int64_t launches0 = ctx.launches;
+    {
+      ScopedPhase ph(ctx, kPhaseSort);
+      do_sort();
+    }
+    step_launches += ctx.launches - launches0;
     return check_launch("sort launch");
   }
 
@@ -505,6 +470,7 @@ struct Sim : SimBase {
     out[PIC_DIAG_POOL_CHUNKS] = (double)pool.n_chunks();
     out[PIC_DIAG_POOL_BYTES] = (double)pool.bytes_held();
     out[PIC_DIAG_LAUNCHES] = (double)ctx.launches;
+    out[PIC_DIAG_STEP_LAUNCHES] = (double)step_launches;
     return PIC_OK;
   }
 
@@ -521,15 +487,18 @@ struct Sim : SimBase {
   }
 
   int enable_timing(int on) override {
-    if (!on && timing) fold_spans();
-    timing = on != 0;
+    if (!on && ctx.timer.on) ctx.timer.fold();
+    ctx.timer.on = on != 0;
     return PIC_OK;
   }
-  int phase_times(float* ms, int reset) override {
+  int phase_times(float* ms, int64_t* launches, int reset) override {
     if (!ms) return fail(PIC_ERR_INVALID_ARG, "null output");
-    fold_spans();
-    for (int i = 0; i < PIC_NPHASE; ++i) ms[i] = phase_ms[i];
-    if (reset) for (int i = 0; i < PIC_NPHASE; ++i) phase_ms[i] = 0;
+    ctx.timer.fold();
+    for (int i = 0; i < PIC_NPHASE; ++i) {
+      ms[i] = ctx.timer.ms[i];
+      if (launches) launches[i] = ctx.timer.count[i];
+    }
+    if (reset) ctx.timer.reset();
     return PIC_OK;
   }
 
@@ -677,9 +646,9 @@ int pic_enable_phase_timing(pic_sim* sim, int32_t on) {
   return sim->impl->enable_timing(on);
 }
 
-int pic_get_phase_times(pic_sim* sim, float* ms, int32_t reset) {
+int pic_get_phase_times(pic_sim* sim, float* ms, int64_t* spans, int32_t reset) {
   SIM_OR_FAIL(sim);
-  return sim->impl->phase_times(ms, reset);
+  return sim->impl->phase_times(ms, spans, reset);
 }
 
 int64_t pic_num_particles(const pic_sim* sim, int32_t species) {
