@@ -65,8 +65,14 @@ enum {
   PIC_DEPOSIT_AUTO = 0,       /* library's choice for the precision / order / sort state */
   PIC_DEPOSIT_GLOBAL = 1,     /* one thread per particle, one global atomic per particle-node
                                  (the paper's GPU design) */
-  PIC_DEPOSIT_COOP = 2        /* warp-cooperative: a warp walks its particles, lanes own window
-                                 nodes, sums held in registers per cell run, one flush per run */
+  PIC_DEPOSIT_COOP = 2,       /* warp-cooperative: a warp walks its particles, lanes own window
+                                 nodes, sums held in registers per cell run, one global
+                                 reduction per node and run */
+  PIC_DEPOSIT_TILE = 3        /* one CTA per sort tile (tile edges <= 8 cells, after the first
+                                 sort; otherwise falls back to COOP / GLOBAL): E/B stencil box
+                                 staged in shared memory for gather + push; deposition by
+                                 16-lane groups into the tile's J box in shared memory, one
+                                 global reduction per node and tile. AUTO picks this when it can. */
 };
 
 /* Options; pass NULL to pic_create for the defaults given here. */

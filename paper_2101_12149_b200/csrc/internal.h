@@ -83,20 +83,30 @@ template <class R> void launch_pack(const Grid<R>& g, const R* valid_src, R* pad
 template <class R> void launch_unpack(const Grid<R>& g, const R* padded_src, R* valid_dst, Ctx& c);
 
 // ---- particles.cu
-enum { kDepositGlobal = 1, kDepositCoop = 2 };
+enum { kDepositGlobal = 1, kDepositCoop = 2, kDepositTile = 3 };
+constexpr int kPushTileThreads = 512;   // k_push_tile: threads per CTA (one CTA per tile)
+constexpr int kDepTileWarps = 12;       // k_deposit_tile: warps per CTA (one CTA per tile)
 template <class R>
 struct ParticleStep {
   Particles<R> cur;                  // x^n, u^{n-1/2}, w
-  Particles<R> alt;                  // the other buffer set: its x,y,z receive x^{n+1} (COOP)
+  Particles<R> alt;                  // the other buffer set: its x,y,z receive x^{n+1} (COOP, TILE)
   const int32_t* cell_sorted;        // cell of every slot at the last sort, or nullptr
-  int32_t* stray_list;               // scratch: indices left to kernel 3 (capacity n)
-  unsigned int* stray_count;
+  const int32_t* tile_start;         // TILE: first slot of every tile (n_tiles + 1 entries)
+  TileSpec tiles;
+  int32_t* stray_list;               // scratch: indices a kernel hands to the next one (capacity n)
+  int32_t* stray_list2;
+  unsigned int* stray_count;         // [0] entries of stray_list, [1] of stray_list2
   unsigned long long* deactivated;
 };
 // One particle step of a species. Returns true if the new positions are in alt.{x,y,z}
 // (the caller swaps the position pointers of the two buffer sets), false if updated in place.
 template <class R>
 bool launch_particles(const Grid<R>& g, const ParticleStep<R>& a, int order, int mode, Ctx& c);
+
+// ---- tile_kernels.cu: k_push_tile + k_deposit_tile of one species (needs tile_start); particles
+// they could not finish are in stray_list / stray_count[0]
+template <class R>
+void launch_tile_kernels(const Grid<R>& g, const ParticleStep<R>& a, int order, Ctx& c);
 
 // ---- sort.cu
 struct SortScratch {
@@ -107,16 +117,18 @@ struct SortScratch {
   int64_t cap = 0;                // particles the buffers are sized for
   int64_t hist_len = 0;
   int64_t scan_len = 0;
-  int32_t* stray_list = nullptr;  // particles.cu: indices handed to the per-particle kernel
-  unsigned int* stray_count = nullptr;
+  int32_t* stray_list = nullptr;  // particles.cu: indices handed from one deposition kernel to the next
+  int32_t* stray_list2 = nullptr;
+  unsigned int* stray_count = nullptr;   // two counters
 };
 int64_t sort_chunk();                                  // keys per block of a radix pass
 int64_t sort_hist_len(int64_t n);                      // entries of `hist` for n particles
 int64_t sort_scan_tmp_len(int64_t hist_len);           // entries of `scan_tmp`
-// Stable sort of `cur` by tile-major cell key into `alt`; fills cell[] and perm[].
+// Stable sort of `cur` by tile-major cell key into `alt`; fills cell[], perm[] and (if not null)
+// tile_start[n_tiles + 1], the first slot of every tile in the new order.
 template <class R>
 void sort_species(const Grid<R>& g, const TileSpec& t, const Particles<R>& cur, const Particles<R>& alt,
-                  int32_t* cell, int32_t* perm, SortScratch& s, Ctx& c);
+                  int32_t* cell, int32_t* perm, int32_t* tile_start, SortScratch& s, Ctx& c);
 
 // ---- diag.cu
 template <class R>

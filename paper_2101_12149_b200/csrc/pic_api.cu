@@ -52,6 +52,7 @@ struct Species {
   int cur = 0;
   int32_t* cell = nullptr;
   int32_t* perm = nullptr;
+  int32_t* tile_start = nullptr;   // n_tiles + 1 entries, valid after a sort
   bool sorted_once = false;
   double q = 0, m = 0;
 };
@@ -189,6 +190,7 @@ struct Sim : SimBase {
     pool.free(scratch.hist);
     pool.free(scratch.scan_tmp);
     pool.free(scratch.stray_list);
+    pool.free(scratch.stray_list2);
     pool.free(scratch.stray_count);
     scratch = SortScratch();
     scratch.hist_len = sort_hist_len(n);
@@ -201,8 +203,9 @@ struct Sim : SimBase {
     scratch.hist = palloc<uint32_t>((size_t)scratch.hist_len);
     scratch.scan_tmp = palloc<uint32_t>((size_t)scratch.scan_len);
     scratch.stray_list = palloc<int32_t>((size_t)n);
-    scratch.stray_count = palloc<unsigned int>(1);
-    if (!scratch.hist || !scratch.scan_tmp || !scratch.stray_list || !scratch.stray_count)
+    scratch.stray_list2 = palloc<int32_t>((size_t)n);
+    scratch.stray_count = palloc<unsigned int>(2);
+    if (!scratch.hist || !scratch.scan_tmp || !scratch.stray_list || !scratch.stray_list2 || !scratch.stray_count)
       return fail(PIC_ERR_OOM, "sort scratch allocation failed");
     scratch.cap = n;
     return PIC_OK;
@@ -219,11 +222,12 @@ struct Sim : SimBase {
     bool ok = alloc_particles(sp.buf[0], n) && alloc_particles(sp.buf[1], n);
     sp.cell = palloc<int32_t>((size_t)(n > 0 ? n : 1));
     sp.perm = palloc<int32_t>((size_t)(n > 0 ? n : 1));
+    sp.tile_start = palloc<int32_t>((size_t)tile.nt[0] * tile.nt[1] * tile.nt[2] + 1);
     auto cleanup = [&]() {
       free_particles(sp.buf[0]); free_particles(sp.buf[1]);
-      pool.free(sp.cell); pool.free(sp.perm);
+      pool.free(sp.cell); pool.free(sp.perm); pool.free(sp.tile_start);
     };
-    if (!ok || !sp.cell || !sp.perm) { cleanup(); return fail(PIC_ERR_OOM, "particle allocation failed"); }
+    if (!ok || !sp.cell || !sp.perm || !sp.tile_start) { cleanup(); return fail(PIC_ERR_OOM, "particle allocation failed"); }
     for (int b = 0; b < 2; ++b) {
       sp.buf[b].kq = (R)(q * dt / (2.0 * m));
       sp.buf[b].jf[0] = (R)(q / (dt * dx[1] * dx[2]));
@@ -299,7 +303,7 @@ struct Sim : SimBase {
   void do_sort() {
     for (auto& sp : species) {
       if (sp.buf[sp.cur].n == 0) { sp.sorted_once = true; continue; }
-      sort_species<R>(g, tile, sp.buf[sp.cur], sp.buf[sp.cur ^ 1], sp.cell, sp.perm, scratch, ctx);
+      sort_species<R>(g, tile, sp.buf[sp.cur], sp.buf[sp.cur ^ 1], sp.cell, sp.perm, sp.tile_start, scratch, ctx);
       sp.cur ^= 1;
       sp.sorted_once = true;
     }
@@ -307,15 +311,20 @@ struct Sim : SimBase {
 
   // AUTO: the warp-cooperative deposition needs the cell-sorted order to pay off
   int pick_mode(const Species<R>& sp) const {
+    const bool tiles_ok = sp.sorted_once && tile.T[0] <= 8 && tile.T[1] <= 8 && tile.T[2] <= 8;
+    if (deposit_mode == PIC_DEPOSIT_TILE && !tiles_ok) return sp.sorted_once ? kDepositCoop : kDepositGlobal;
     if (deposit_mode != PIC_DEPOSIT_AUTO) return deposit_mode;
-    return sp.sorted_once ? kDepositCoop : kDepositGlobal;
+    return tiles_ok ? kDepositTile : (sp.sorted_once ? kDepositCoop : kDepositGlobal);
   }
   void particle_step(Species<R>& sp) {
     ParticleStep<R> a;
     a.cur = sp.buf[sp.cur];
     a.alt = sp.buf[sp.cur ^ 1];
     a.cell_sorted = sp.sorted_once ? sp.cell : nullptr;
+    a.tile_start = sp.tile_start;
+    a.tiles = tile;
     a.stray_list = scratch.stray_list;
+    a.stray_list2 = scratch.stray_list2;
     a.stray_count = scratch.stray_count;
     a.deactivated = d_deact;
     if (launch_particles<R>(g, a, order, pick_mode(sp), ctx)) {
@@ -542,7 +551,7 @@ int pic_create(const int32_t n_cells[3], const double dx[3], double dt, int shap
   if (shape_order < 1 || shape_order > 3) return bad(PIC_ERR_INVALID_ARG, "shape_order must be 1, 2 or 3");
   if (prec != PIC_F64 && prec != PIC_F32) return bad(PIC_ERR_INVALID_ARG, "unknown precision");
   if (o.sort_interval < 0 || o.sort_key_mode < 0 || o.sort_key_mode > 1 || o.reserved != 0 || o.deposit_mode < 0 ||
-      o.deposit_mode > 2)
+      o.deposit_mode > 3)
     return bad(PIC_ERR_INVALID_ARG, "bad option value");
   double s2 = 0;
   for (int d = 0; d < 3; ++d) {

@@ -194,6 +194,20 @@ __global__ void __launch_bounds__(256) k_permute(Grid<R> g, Particles<R> src, Pa
   cell[k] = cx + g.N[0] * (cy + g.N[1] * cz);
 }
 
+// ---- first slot of every tile in the sorted order (tile-major key): tile_start[t] = first k with
+// tile(key[k]) >= t, tile_start[n_tiles] = n. Written without atomics: the thread at a tile
+// boundary fills the entries of every tile that begins there (empty tiles included).
+__global__ void __launch_bounds__(256) k_tile_bounds(const uint32_t* __restrict__ keys, int64_t n, uint32_t tvol,
+                                                     int n_tiles, int32_t* __restrict__ tile_start) {
+  int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  int tk = (int)(keys[k] / tvol);
+  int tp = k == 0 ? -1 : (int)(keys[k - 1] / tvol);
+  for (int t = tp + 1; t <= tk; ++t) tile_start[t] = (int32_t)k;
+  if (k == n - 1)
+    for (int t = tk + 1; t <= n_tiles; ++t) tile_start[t] = (int32_t)n;
+}
+
 int key_bits(const TileSpec& t) {
   uint64_t nb = (uint64_t)t.nt[0] * t.nt[1] * t.nt[2] * (t.key_mode == 0 ? (uint64_t)t.tvol : 1ull);
   int b = 0;
@@ -217,7 +231,7 @@ int64_t sort_scan_tmp_len(int64_t hist_len) {
 
 template <class R>
 void sort_species(const Grid<R>& g, const TileSpec& t, const Particles<R>& cur, const Particles<R>& alt,
-                  int32_t* cell, int32_t* perm, SortScratch& s, Ctx& c) {
+                  int32_t* cell, int32_t* perm, int32_t* tile_start, SortScratch& s, Ctx& c) {
   const int64_t n = cur.n;
   if (n == 0) return;
   const int nblocks = (int)((n + kSortChunk - 1) / kSortChunk);
@@ -236,11 +250,17 @@ void sort_species(const Grid<R>& g, const TileSpec& t, const Particles<R>& cur, 
   }
   k_permute<R><<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(g, cur, alt, s.vals[in], cell, perm);
   c.launches++;
+  if (tile_start) {
+    const uint32_t tvol = t.key_mode == 0 ? (uint32_t)t.tvol : 1u;
+    k_tile_bounds<<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(s.keys[in], n, tvol, t.nt[0] * t.nt[1] * t.nt[2],
+                                                                   tile_start);
+    c.launches++;
+  }
 }
 
 template void sort_species<double>(const Grid<double>&, const TileSpec&, const Particles<double>&,
-                                   const Particles<double>&, int32_t*, int32_t*, SortScratch&, Ctx&);
+                                   const Particles<double>&, int32_t*, int32_t*, int32_t*, SortScratch&, Ctx&);
 template void sort_species<float>(const Grid<float>&, const TileSpec&, const Particles<float>&,
-                                  const Particles<float>&, int32_t*, int32_t*, SortScratch&, Ctx&);
+                                  const Particles<float>&, int32_t*, int32_t*, int32_t*, SortScratch&, Ctx&);
 
 }  // namespace pic

@@ -1,0 +1,395 @@
+// Tile-centric particle kernels: one CTA per particle tile (<= 8x8x8 cells,
+// the bins of the sort). After a sort the particles of a tile are one contiguous
+// range [tile_start[t], tile_start[t+1]) in cell order, which gives both kernels their locality:
+//   k_push_tile     stages the tile's E/B stencil box in shared memory once, then gathers and
+//                   pushes one particle per thread from it (gather + push fused, no
+//                   per-particle E/B in memory);
+//   k_deposit_tile  Esirkepov deposition (ref [8]) by groups of 16 lanes (4 at
+//                   order 1): the lanes of a group own the (j,k) columns of a cell's window, x runs
+//                   along registers, sums stay in registers for a run of cells along x, are folded
+//                   into the tile's J box in shared memory, and reach global memory once per tile.
+// Particles that no longer fit the tile's boxes (they drifted since the last sort) are handled by
+// the global-memory paths in particles.cu; correctness never depends on the order or the tile.
+#include <climits>
+
+#include "internal.h"
+#include "particle_math.cuh"
+
+namespace pic {
+
+namespace {
+
+constexpr int kTileMax = 8;   // largest tile edge (cells) these kernels are laid out for
+
+__device__ __forceinline__ void tile_coords(const TileSpec& ts, int tile, int* tb) {
+  int tx = tile % ts.nt[0];
+  int r = tile / ts.nt[0];
+  int ty = r % ts.nt[1];
+  int tz = r / ts.nt[1];
+  tb[0] = tx * ts.T[0];
+  tb[1] = ty * ts.T[1];
+  tb[2] = tz * ts.T[2];
+}
+
+// =================================================================== gather + push from shared memory
+// Box of nodes staged per component: local index 0 is node (tile base - HB); EXT nodes per axis cover
+// the stencils (nodal and staggered) of every particle whose cell is within one cell of the tile.
+template <int ORDER>
+struct PushBox {
+  static constexpr int HB = ORDER == 3 ? 3 : 2;
+  static constexpr int EXT = kTileMax + (ORDER == 1 ? 4 : (ORDER == 2 ? 5 : 6));   // 12, 13, 14
+  static constexpr int VOL = EXT * EXT * EXT;
+};
+
+template <class R, int ORDER>
+__device__ __forceinline__ R interp_box(const R* __restrict__ F, int base, const R* wx, const R* wy, const R* wz) {
+  constexpr int E = PushBox<ORDER>::EXT;
+  R acc = 0;
+#pragma unroll
+  for (int c = 0; c <= ORDER; ++c) {
+    R accb = 0;
+#pragma unroll
+    for (int b = 0; b <= ORDER; ++b) {
+      R acca = 0;
+#pragma unroll
+      for (int a = 0; a <= ORDER; ++a) acca += wx[a] * F[base + a + E * b + E * E * c];
+      accb += wy[b] * acca;
+    }
+    acc += wz[c] * accb;
+  }
+  return acc;
+}
+
+template <class R, int ORDER>
+__global__ void __launch_bounds__(kPushTileThreads) k_push_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn,
+                                                                R* __restrict__ yn, R* __restrict__ zn,
+                                                                const int32_t* __restrict__ tile_start, TileSpec ts) {
+  using PB = PushBox<ORDER>;
+  constexpr int E = PB::EXT, VOL = PB::VOL;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  R* box = reinterpret_cast<R*>(smem_raw);   // [6][E][E][E]
+  const int tile = blockIdx.x;
+  const int s = tile_start[tile], e = tile_start[tile + 1];
+  if (s >= e) return;
+  int tb[3];
+  tile_coords(ts, tile, tb);
+  const int o0 = tb[0] - PB::HB, o1 = tb[1] - PB::HB, o2 = tb[2] - PB::HB;   // node of local (0,0,0)
+  // stage the six boxes (nodes beyond the padded array, possible only for tiles smaller than 8, read 0)
+  const int lim0 = g.N[0] + kGuard, lim1 = g.N[1] + kGuard, lim2 = g.N[2] + kGuard;
+  for (int idx = threadIdx.x; idx < VOL; idx += blockDim.x) {
+    int i = idx % E, r = idx / E;
+    int j = r % E, k = r / E;
+    const bool in = (o0 + i < lim0) & (o1 + j < lim1) & (o2 + k < lim2);
+    const int gi = g.idx(o0 + i, o1 + j, o2 + k);
+#pragma unroll
+    for (int c = 0; c < 6; ++c) box[c * VOL + idx] = in ? __ldg(g.F[c] + gi) : R(0);
+  }
+  __syncthreads();
+  for (int t = s + threadIdx.x; t < e; t += blockDim.x) {
+    R x0[3] = {p.x[t], p.y[t], p.z[t]};
+    R u[3] = {p.ux[t], p.uy[t], p.uz[t]};
+    R wn[3][ORDER + 1], ws[3][ORDER + 1];
+    int ln[3], ls[3];
+    bool inbox = true;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      R xi = x0[d] * g.inv_dx[d];
+      ln[d] = shape<R, ORDER>(xi, wn[d]);
+      ls[d] = shape<R, ORDER>(xi - R(0.5), ws[d]);
+      const int od = d == 0 ? o0 : (d == 1 ? o1 : o2);
+      const int a = ln[d] - od, b = ls[d] - od;
+      inbox &= (a >= 0) & (a <= E - ORDER - 1) & (b >= 0) & (b <= E - ORDER - 1);
+      if (inbox) { ln[d] = a; ls[d] = b; }
+    }
+    R Ef[3], Bf[3];
+    if (inbox) {
+      // Ex (s,n,n)  Ey (n,s,n)  Ez (n,n,s)  Bx (n,s,s)  By (s,n,s)  Bz (s,s,n)
+      Ef[0] = interp_box<R, ORDER>(box + 0 * VOL, ls[0] + E * (ln[1] + E * ln[2]), ws[0], wn[1], wn[2]);
+      Ef[1] = interp_box<R, ORDER>(box + 1 * VOL, ln[0] + E * (ls[1] + E * ln[2]), wn[0], ws[1], wn[2]);
+      Ef[2] = interp_box<R, ORDER>(box + 2 * VOL, ln[0] + E * (ln[1] + E * ls[2]), wn[0], wn[1], ws[2]);
+      Bf[0] = interp_box<R, ORDER>(box + 3 * VOL, ln[0] + E * (ls[1] + E * ls[2]), wn[0], ws[1], ws[2]);
+      Bf[1] = interp_box<R, ORDER>(box + 4 * VOL, ls[0] + E * (ln[1] + E * ls[2]), ws[0], wn[1], ws[2]);
+      Bf[2] = interp_box<R, ORDER>(box + 5 * VOL, ls[0] + E * (ls[1] + E * ln[2]), ws[0], ws[1], wn[2]);
+    } else {
+      gather6<R, ORDER>(g, x0[0], x0[1], x0[2], Ef, Bf);   // drifted out of the box: global memory
+    }
+    boris<R>(p.kq, g.inv_c2, Ef, Bf, u);
+    R ig = g.dt / sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * g.inv_c2);
+    xn[t] = x0[0] + u[0] * ig;
+    yn[t] = x0[1] + u[1] * ig;
+    zn[t] = x0[2] + u[2] * ig;
+    p.ux[t] = u[0]; p.uy[t] = u[1]; p.uz[t] = u[2];
+  }
+}
+
+// =================================================================== Esirkepov deposition per tile
+template <class R>
+struct alignas(2 * sizeof(R)) Pair2 { R a, b; };
+
+// Windows fixed to a CELL c (the cell of the old position): x nodes c-BLX .. c-BLX+NX-1 cover any
+// move of up to one cell along x; y and z nodes c-BLYZ .. c-BLYZ+NYZ-1 cover the moves that stay in
+// the cell along that axis (the others go to the list). NYZ^2 lanes own the (j,k) columns.
+template <int ORDER>
+struct TWin {
+  static constexpr int NX = ORDER == 1 ? 4 : 6, BLX = ORDER == 1 ? 1 : 2;
+  static constexpr int NYZ = ORDER == 1 ? 2 : 4, BLYZ = ORDER == 1 ? 0 : 1;
+  static constexpr int LG = NYZ * NYZ;                 // lanes per particle: 4 or 16
+  static constexpr int EX = kTileMax + NX - 1;         // J box of the tile: 11 / 13 nodes along x
+  static constexpr int EYZ = kTileMax + NYZ - 1;       // 9 / 11 along y and z
+  static constexpr int JVOL = EX * EYZ * EYZ;
+  // record (elements): {A_x,B_x}[NX] | PX[NX] | {S0_y,DS_y}[NYZ] | PY[NYZ] | {S0_z,DS_z}[NYZ] | PZ[NYZ]
+  static constexpr int oAB = 0, oPX = 2 * NX, oY = 3 * NX, oPY = 3 * NX + 2 * NYZ, oZ = 3 * NX + 3 * NYZ,
+                       oPZ = 3 * NX + 5 * NYZ;
+  static constexpr int RAW = 3 * NX + 6 * NYZ;                     // 42 / 24
+  static constexpr int REC = (RAW / 2) % 2 == 1 ? RAW : RAW + 2;   // REC/2 odd: conflict-free pair stores
+};
+
+// old/new weights of one axis placed on an NW-node window whose first node is (cell - BL);
+// `fits` = both supports lie inside the window
+template <class R, int ORDER, int NW, int BL>
+__device__ __forceinline__ void axis_window(R xi0, R xi1, int N, int& cell, R* S0, R* DS, bool& fits) {
+  R w0[ORDER + 1], w1[ORDER + 1];
+  int l0 = shape<R, ORDER>(xi0, w0);
+  int l1 = shape<R, ORDER>(xi1, w1);
+  int c = ORDER == 2 ? (int)floor(xi0) : (ORDER == 1 ? l0 : l0 + 1);
+  c = min(max(c, 0), N);
+  const int so0 = l0 - (c - BL), sl1 = l1 - (c - BL);
+#pragma unroll
+  for (int i = 0; i < NW; ++i) {
+    R a = 0, b = 0;
+#pragma unroll
+    for (int k = 0; k <= ORDER; ++k) {
+      a = (i == so0 + k) ? w0[k] : a;
+      b = (i == sl1 + k) ? w1[k] : b;
+    }
+    S0[i] = a;
+    DS[i] = b - a;
+  }
+  fits = (so0 >= 0) & (so0 + ORDER < NW) & (sl1 >= 0) & (sl1 + ORDER < NW);
+  cell = c;
+}
+
+__device__ __forceinline__ void smem_add(double* p, double v) { atomicAdd(p, v); }   // CAS loop on sm_100a
+__device__ __forceinline__ void smem_add(float* p, float v) { atomicAdd(p, v); }
+
+template <class R, int ORDER>
+__global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn,
+                                                                     R* __restrict__ yn, R* __restrict__ zn,
+                                                                     const int32_t* __restrict__ tile_start, TileSpec ts,
+                                                                     int32_t* __restrict__ stray_list,
+                                                                     unsigned int* __restrict__ stray_count,
+                                                                     unsigned long long* deactivated) {
+  using W = TWin<ORDER>;
+  constexpr int NX = W::NX, NYZ = W::NYZ, LG = W::LG, EX = W::EX, EYZ = W::EYZ, JVOL = W::JVOL, REC = W::REC;
+  constexpr int GPW = 32 / LG;                       // groups per warp
+  constexpr int NGRP = kDepTileWarps * GPW;          // groups per CTA
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  R* Jt = reinterpret_cast<R*>(smem_raw);            // [3][EYZ][EYZ][EX]
+  R* rec_all = Jt + 3 * JVOL + ((3 * JVOL) & 1);     // keep 16-byte alignment of the records
+  __shared__ int s_ib[kDepTileWarps][32];
+
+  const int tile = blockIdx.x;
+  const int s = tile_start[tile], e = tile_start[tile + 1];
+  if (s >= e) return;
+  int tb[3];
+  tile_coords(ts, tile, tb);
+  for (int i = threadIdx.x; i < 3 * JVOL; i += blockDim.x) Jt[i] = R(0);
+  __syncthreads();
+
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int grp = lane / LG, gl = lane % LG;
+  const int j = gl % NYZ, k = gl / NYZ;
+  const int off_jk = EX * (j + EYZ * k);
+  R* rec = rec_all + (size_t)warp * 32 * REC;
+  const R half = R(0.5), third = R(1) / R(3);
+
+  const int n = e - s;
+  const int chunk = ((n + NGRP - 1) / NGRP + LG - 1) / LG * LG;   // particles per group, multiple of LG
+  const int gb = s + (warp * GPW + grp) * chunk;
+  const int ge = min(e, gb + chunk);
+  const int rounds = chunk / LG;
+
+  R ax[NX - 1], ay[NX], az[NX];
+#pragma unroll
+  for (int i = 0; i < NX; ++i) { ay[i] = 0; az[i] = 0; if (i < NX - 1) ax[i] = 0; }
+  int cur = INT_MIN;   // J-box offset of the window base of the run being accumulated
+
+  auto flush_all = [&]() {
+    if (cur == INT_MIN) return;
+    R* jx = Jt + cur + off_jk;
+#pragma unroll
+    for (int i = 0; i < NX; ++i) {
+      if (i < NX - 1 && ax[i] != R(0)) smem_add(jx + i, ax[i]);
+      if (ay[i] != R(0)) smem_add(jx + JVOL + i, ay[i]);
+      if (az[i] != R(0)) smem_add(jx + 2 * JVOL + i, az[i]);
+    }
+  };
+  auto shift_one = [&]() {   // the run moves one cell up in x: x-slot 0 is complete
+    R* jx = Jt + cur + off_jk;
+    if (ax[0] != R(0)) smem_add(jx, ax[0]);
+    if (ay[0] != R(0)) smem_add(jx + JVOL, ay[0]);
+    if (az[0] != R(0)) smem_add(jx + 2 * JVOL, az[0]);
+#pragma unroll
+    for (int i = 0; i < NX - 1; ++i) { ay[i] = ay[i + 1]; az[i] = az[i + 1]; if (i < NX - 2) ax[i] = ax[i + 1]; }
+    ay[NX - 1] = 0; az[NX - 1] = 0; ax[NX - 2] = 0;
+    cur += 1;
+  };
+
+  for (int r = 0; r < rounds; ++r) {
+    const int t = gb + r * LG + gl;
+    const bool valid = t < ge;
+    bool elig = false;
+    R x1[3] = {0, 0, 0};
+    R w = 0;
+    if (valid) {
+      R x0[3] = {p.x[t], p.y[t], p.z[t]};
+      x1[0] = xn[t]; x1[1] = yn[t]; x1[2] = zn[t];
+      w = p.w[t];
+      R S0x[NX], DSx[NX], S0y[NYZ], DSy[NYZ], S0z[NYZ], DSz[NYZ];
+      int c[3];
+      bool fit[3];
+      axis_window<R, ORDER, NX, W::BLX>(x0[0] * g.inv_dx[0], x1[0] * g.inv_dx[0], g.N[0], c[0], S0x, DSx, fit[0]);
+      axis_window<R, ORDER, NYZ, W::BLYZ>(x0[1] * g.inv_dx[1], x1[1] * g.inv_dx[1], g.N[1], c[1], S0y, DSy, fit[1]);
+      axis_window<R, ORDER, NYZ, W::BLYZ>(x0[2] * g.inv_dx[2], x1[2] * g.inv_dx[2], g.N[2], c[2], S0z, DSz, fit[2]);
+      const int rc0 = c[0] - tb[0], rc1 = c[1] - tb[1], rc2 = c[2] - tb[2];
+      elig = fit[0] & fit[1] & fit[2] & (rc0 >= 0) & (rc0 < ts.T[0]) & (rc1 >= 0) & (rc1 < ts.T[1]) & (rc2 >= 0) &
+             (rc2 < ts.T[2]);
+      if (elig) {
+        s_ib[warp][lane] = rc0 + EX * (rc1 + EYZ * rc2);
+        R* rr = rec + lane * REC;
+        const R fx = -(w * p.jf[0]), fy = -(w * p.jf[1]), fz = -(w * p.jf[2]);
+        R px = 0, py = 0, pz = 0;
+#pragma unroll
+        for (int i = 0; i < NX; ++i) {
+          *reinterpret_cast<Pair2<R>*>(rr + W::oAB + 2 * i) =
+              Pair2<R>{S0x[i] + half * DSx[i], half * S0x[i] + third * DSx[i]};
+          px += DSx[i];
+          rr[W::oPX + i] = fx * px;
+        }
+#pragma unroll
+        for (int i = 0; i < NYZ; ++i) {
+          *reinterpret_cast<Pair2<R>*>(rr + W::oY + 2 * i) = Pair2<R>{S0y[i], DSy[i]};
+          *reinterpret_cast<Pair2<R>*>(rr + W::oZ + 2 * i) = Pair2<R>{S0z[i], DSz[i]};
+          py += DSy[i]; pz += DSz[i];
+          rr[W::oPY + i] = fy * py;
+          rr[W::oPZ + i] = fz * pz;
+        }
+      }
+    }
+    __syncwarp();
+    const unsigned bal = __ballot_sync(0xffffffffu, elig);
+    const unsigned gm = (bal >> (grp * LG)) & (LG == 32 ? 0xffffffffu : ((1u << LG) - 1u));
+#pragma unroll 1
+    for (int q = 0; q < LG; ++q) {
+      if (!((gm >> q) & 1u)) continue;
+      const int src = grp * LG + q;
+      const int ibq = s_ib[warp][src];
+      if (ibq != cur) {
+        const int sh = ibq - cur;
+        if (cur != INT_MIN && sh > 0 && sh < NX) {
+          for (int i = 0; i < sh; ++i) shift_one();
+        } else {
+          flush_all();
+#pragma unroll
+          for (int i = 0; i < NX; ++i) { ay[i] = 0; az[i] = 0; if (i < NX - 1) ax[i] = 0; }
+          cur = ibq;
+        }
+      }
+      const R* rr = rec + src * REC;
+      const Pair2<R> yv = *reinterpret_cast<const Pair2<R>*>(rr + W::oY + 2 * j);
+      const Pair2<R> zv = *reinterpret_cast<const Pair2<R>*>(rr + W::oZ + 2 * k);
+      const R py = rr[W::oPY + j], pz = rr[W::oPZ + k];
+      const R cx = zv.a * (yv.a + half * yv.b) + zv.b * (half * yv.a + third * yv.b);
+      const R q1 = py * zv.a, q2 = py * zv.b;
+      const R r1 = pz * yv.a, r2 = pz * yv.b;
+#pragma unroll
+      for (int i = 0; i < NX; ++i) {
+        const Pair2<R> ab = *reinterpret_cast<const Pair2<R>*>(rr + W::oAB + 2 * i);
+        if (i < NX - 1) ax[i] += cx * rr[W::oPX + i];
+        ay[i] += q1 * ab.a + q2 * ab.b;
+        az[i] += r1 * ab.a + r2 * ab.b;
+      }
+    }
+    __syncwarp();
+    // particles deposited here are finished: wrap and store; the others go to the list untouched
+    const bool stray = valid && !elig;
+    const unsigned sm = __ballot_sync(0xffffffffu, stray);
+    if (sm) {
+      unsigned base = 0;
+      if (lane == 0) base = atomicAdd(stray_count, (unsigned)__popc(sm));
+      base = __shfl_sync(0xffffffffu, base, 0);
+      if (stray) stray_list[base + __popc(sm & ((1u << lane) - 1u))] = (int32_t)t;
+    }
+    if (valid && elig) {
+      bool out = false;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) out |= wrap_axis<R>(x1[d], g.L[d], g.periodic[d]);
+      if (out) {
+        if (w != R(0)) atomicAdd(deactivated, 1ull);
+        p.w[t] = R(0);
+      }
+      xn[t] = x1[0]; yn[t] = x1[1]; zn[t] = x1[2];
+    }
+  }
+  flush_all();
+  __syncthreads();
+  // the tile's J box -> global memory, one reduction per touched node
+  const int b0 = tb[0] - W::BLX, b1 = tb[1] - W::BLYZ, b2 = tb[2] - W::BLYZ;
+  for (int idx = threadIdx.x; idx < JVOL; idx += blockDim.x) {
+    const int i = idx % EX, rr = idx / EX;
+    const int jj = rr % EYZ, kk = rr / EYZ;
+    const int gi = g.idx(b0 + i, b1 + jj, b2 + kk);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const R v = Jt[c * JVOL + idx];
+      if (v != R(0)) red_add(g.J[c] + gi, v);
+    }
+  }
+}
+
+}  // namespace
+
+template <int ORDER, class R>
+static size_t dep_smem_bytes() {
+  using W = TWin<ORDER>;
+  return (size_t)(3 * W::JVOL + ((3 * W::JVOL) & 1) + kDepTileWarps * 32 * W::REC) * sizeof(R);
+}
+
+template <class R, int ORDER>
+static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, Ctx& c) {
+  const Particles<R>& p = a.cur;
+  R *xn = a.alt.x, *yn = a.alt.y, *zn = a.alt.z;
+  const int n_tiles = a.tiles.nt[0] * a.tiles.nt[1] * a.tiles.nt[2];
+  static bool attr_set = false;
+  const size_t push_smem = (size_t)6 * PushBox<ORDER>::VOL * sizeof(R);
+  const size_t dep_smem = dep_smem_bytes<ORDER, R>();
+  if (!attr_set) {
+    cudaFuncSetAttribute(k_push_tile<R, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
+    cudaFuncSetAttribute(k_deposit_tile<R, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dep_smem);
+    attr_set = true;
+  }
+  {
+    ScopedPhase ph(c, kPhasePush);
+    k_push_tile<R, ORDER><<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles);
+  }
+  {
+    ScopedPhase ph(c, kPhaseDeposit);
+    k_deposit_tile<R, ORDER><<<n_tiles, kDepTileWarps * 32, dep_smem, c.stream>>>(
+        g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list, a.stray_count, a.deactivated);
+  }
+  c.launches += 2;
+}
+
+template <class R>
+void launch_tile_kernels(const Grid<R>& g, const ParticleStep<R>& a, int order, Ctx& c) {
+  switch (order) {
+    case 1: launch_tile_order<R, 1>(g, a, c); break;
+    case 2: launch_tile_order<R, 2>(g, a, c); break;
+    default: launch_tile_order<R, 3>(g, a, c); break;
+  }
+}
+
+template void launch_tile_kernels<double>(const Grid<double>&, const ParticleStep<double>&, int, Ctx&);
+template void launch_tile_kernels<float>(const Grid<float>&, const ParticleStep<float>&, int, Ctx&);
+
+}  // namespace pic
