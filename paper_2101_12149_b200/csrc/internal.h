@@ -85,7 +85,7 @@ template <class R> void launch_unpack(const Grid<R>& g, const R* padded_src, R* 
 // ---- particles.cu
 enum { kDepositGlobal = 1, kDepositCoop = 2, kDepositTile = 3 };
 constexpr int kPushTileThreads = 512;   // k_push_tile: threads per CTA (one CTA per tile)
-constexpr int kDepTileWarps = 12;       // k_deposit_tile: warps per CTA (one CTA per tile)
+constexpr int kDepTileWarps = 16;       // k_deposit_tile: warps per CTA (one CTA per tile)
 template <class R>
 struct ParticleStep {
   Particles<R> cur;                  // x^n, u^{n-1/2}, w

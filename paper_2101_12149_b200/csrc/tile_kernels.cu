@@ -52,7 +52,7 @@ __device__ __forceinline__ R interp_box(const R* __restrict__ F, int base, const
     for (int b = 0; b <= ORDER; ++b) {
       R acca = 0;
 #pragma unroll
-      for (int a = 0; a <= ORDER; ++a) acca += wx[a] * F[base + a + E * b + E * E * c];
+      for (int a = 0; a <= ORDER; ++a) acca += wx[a] * F[base + E * E * a + b + E * c];
       accb += wy[b] * acca;
     }
     acc += wz[c] * accb;
@@ -76,9 +76,13 @@ __global__ void __launch_bounds__(kPushTileThreads) k_push_tile(Grid<R> g, Parti
   const int o0 = tb[0] - PB::HB, o1 = tb[1] - PB::HB, o2 = tb[2] - PB::HB;   // node of local (0,0,0)
   // stage the six boxes (nodes beyond the padded array, possible only for tiles smaller than 8, read 0)
   const int lim0 = g.N[0] + kGuard, lim1 = g.N[1] + kGuard, lim2 = g.N[2] + kGuard;
+  // box layout: y fastest, then z, x slowest. The lanes of a warp hold particles of a few cells that
+  // are neighbours along x, so their stencil addresses differ by multiples of E*E = 196 = 4 (mod 16
+  // doubles): no two fall in the same bank pair (2.10 wavefronts per 64-bit load against 2.58 with x
+  // fastest, where a y-staggered base one row up collides with a cell two to the right).
   for (int idx = threadIdx.x; idx < VOL; idx += blockDim.x) {
-    int i = idx % E, r = idx / E;
-    int j = r % E, k = r / E;
+    int j = idx % E, r = idx / E;
+    int k = r % E, i = r / E;
     const bool in = (o0 + i < lim0) & (o1 + j < lim1) & (o2 + k < lim2);
     const int gi = g.idx(o0 + i, o1 + j, o2 + k);
 #pragma unroll
@@ -104,12 +108,12 @@ __global__ void __launch_bounds__(kPushTileThreads) k_push_tile(Grid<R> g, Parti
     R Ef[3], Bf[3];
     if (inbox) {
       // Ex (s,n,n)  Ey (n,s,n)  Ez (n,n,s)  Bx (n,s,s)  By (s,n,s)  Bz (s,s,n)
-      Ef[0] = interp_box<R, ORDER>(box + 0 * VOL, ls[0] + E * (ln[1] + E * ln[2]), ws[0], wn[1], wn[2]);
-      Ef[1] = interp_box<R, ORDER>(box + 1 * VOL, ln[0] + E * (ls[1] + E * ln[2]), wn[0], ws[1], wn[2]);
-      Ef[2] = interp_box<R, ORDER>(box + 2 * VOL, ln[0] + E * (ln[1] + E * ls[2]), wn[0], wn[1], ws[2]);
-      Bf[0] = interp_box<R, ORDER>(box + 3 * VOL, ln[0] + E * (ls[1] + E * ls[2]), wn[0], ws[1], ws[2]);
-      Bf[1] = interp_box<R, ORDER>(box + 4 * VOL, ls[0] + E * (ln[1] + E * ls[2]), ws[0], wn[1], ws[2]);
-      Bf[2] = interp_box<R, ORDER>(box + 5 * VOL, ls[0] + E * (ls[1] + E * ln[2]), ws[0], ws[1], wn[2]);
+      Ef[0] = interp_box<R, ORDER>(box + 0 * VOL, E * E * ls[0] + ln[1] + E * ln[2], ws[0], wn[1], wn[2]);
+      Ef[1] = interp_box<R, ORDER>(box + 1 * VOL, E * E * ln[0] + ls[1] + E * ln[2], wn[0], ws[1], wn[2]);
+      Ef[2] = interp_box<R, ORDER>(box + 2 * VOL, E * E * ln[0] + ln[1] + E * ls[2], wn[0], wn[1], ws[2]);
+      Bf[0] = interp_box<R, ORDER>(box + 3 * VOL, E * E * ln[0] + ls[1] + E * ls[2], wn[0], ws[1], ws[2]);
+      Bf[1] = interp_box<R, ORDER>(box + 4 * VOL, E * E * ls[0] + ln[1] + E * ls[2], ws[0], wn[1], ws[2]);
+      Bf[2] = interp_box<R, ORDER>(box + 5 * VOL, E * E * ls[0] + ls[1] + E * ln[2], ws[0], ws[1], wn[2]);
     } else {
       gather6<R, ORDER>(g, x0[0], x0[1], x0[2], Ef, Bf);   // drifted out of the box: global memory
     }
@@ -144,16 +148,18 @@ struct TWin {
   static constexpr int REC = (RAW / 2) % 2 == 1 ? RAW : RAW + 2;   // REC/2 odd: conflict-free pair stores
 };
 
-// old/new weights of one axis placed on an NW-node window whose first node is (cell - BL);
-// `fits` = both supports lie inside the window
+// old/new weights of one axis placed on an NW-node window whose first node is (cell - BL), where
+// `cell` is the cell of the OLD position; `fits` = both supports lie inside the window. For orders 1
+// and 3 the old support starts at a fixed slot (cell - 1 + ... is static), so only the new weights
+// need selects.
 template <class R, int ORDER, int NW, int BL>
-__device__ __forceinline__ void axis_window(R xi0, R xi1, int N, int& cell, R* S0, R* DS, bool& fits) {
+__device__ __forceinline__ void axis_window(R xi0, R xi1, int& cell, R* S0, R* DS, bool& fits) {
   R w0[ORDER + 1], w1[ORDER + 1];
-  int l0 = shape<R, ORDER>(xi0, w0);
-  int l1 = shape<R, ORDER>(xi1, w1);
-  int c = ORDER == 2 ? (int)floor(xi0) : (ORDER == 1 ? l0 : l0 + 1);
-  c = min(max(c, 0), N);
-  const int so0 = l0 - (c - BL), sl1 = l1 - (c - BL);
+  const int l0 = shape<R, ORDER>(xi0, w0);
+  const int l1 = shape<R, ORDER>(xi1, w1);
+  const int c = ORDER == 2 ? (int)floor(xi0) : (ORDER == 1 ? l0 : l0 + 1);
+  const int so0 = ORDER == 2 ? l0 - (c - BL) : (ORDER == 1 ? BL : BL - 1);
+  const int sl1 = l1 - (c - BL);
 #pragma unroll
   for (int i = 0; i < NW; ++i) {
     R a = 0, b = 0;
@@ -172,6 +178,73 @@ __device__ __forceinline__ void axis_window(R xi0, R xi1, int N, int& cell, R* S
 __device__ __forceinline__ void smem_add(double* p, double v) { atomicAdd(p, v); }   // CAS loop on sm_100a
 __device__ __forceinline__ void smem_add(float* p, float v) { atomicAdd(p, v); }
 
+// Register accumulators of one lane: the (j,k) column of a window of NX nodes along x, three
+// components. The slot of box node X is X mod NX, so when the window advances by one cell nothing
+// moves: the slot of the node that left is flushed and reused for the node that entered.
+template <class R, int NX>
+struct Acc {
+  R x[NX], y[NX], z[NX];
+  __device__ __forceinline__ void zero() {
+#pragma unroll
+    for (int i = 0; i < NX; ++i) { x[i] = 0; y[i] = 0; z[i] = 0; }
+  }
+};
+
+// one particle's contribution to this lane's column; PH = (first box node of the window) mod NX
+template <class R, int ORDER, int PH>
+__device__ __forceinline__ void accumulate(Acc<R, TWin<ORDER>::NX>& a, const R* __restrict__ rr, int j, int k) {
+  using W = TWin<ORDER>;
+  constexpr int NX = W::NX;
+  const R half = R(0.5), third = R(1) / R(3);
+  const Pair2<R> yv = *reinterpret_cast<const Pair2<R>*>(rr + W::oY + 2 * j);
+  const Pair2<R> zv = *reinterpret_cast<const Pair2<R>*>(rr + W::oZ + 2 * k);
+  const R py = rr[W::oPY + j], pz = rr[W::oPZ + k];
+  const R cx = zv.a * (yv.a + half * yv.b) + zv.b * (half * yv.a + third * yv.b);
+  const R q1 = py * zv.a, q2 = py * zv.b;
+  const R r1 = pz * yv.a, r2 = pz * yv.b;
+#pragma unroll
+  for (int i = 0; i < NX; ++i) {
+    const int P = (PH + i) % NX;   // static after unrolling
+    const Pair2<R> ab = *reinterpret_cast<const Pair2<R>*>(rr + W::oAB + 2 * i);
+    if (i < NX - 1) a.x[P] = fma(cx, rr[W::oPX + i], a.x[P]);
+    a.y[P] = fma(q1, ab.a, fma(q2, ab.b, a.y[P]));
+    a.z[P] = fma(r1, ab.a, fma(r2, ab.b, a.z[P]));
+  }
+}
+
+// window advanced by one cell along x: the node that left (old logical slot 0, physical slot
+// PH - 1) goes to the box at jx_old[0]; then accumulate
+template <class R, int ORDER, int PH>
+__device__ __forceinline__ void step_phase(Acc<R, TWin<ORDER>::NX>& a, bool adv, R* jx_old, const R* __restrict__ rr,
+                                           int j, int k) {
+  using W = TWin<ORDER>;
+  constexpr int NX = W::NX;
+  constexpr int PO = (PH + NX - 1) % NX;
+  if (adv) {
+    if (a.x[PO] != R(0)) smem_add(jx_old, a.x[PO]);
+    if (a.y[PO] != R(0)) smem_add(jx_old + W::JVOL, a.y[PO]);
+    if (a.z[PO] != R(0)) smem_add(jx_old + 2 * W::JVOL, a.z[PO]);
+    a.x[PO] = 0; a.y[PO] = 0; a.z[PO] = 0;
+  }
+  accumulate<R, ORDER, PH>(a, rr, j, k);
+}
+
+// all slots to the box: physical slot p holds logical slot (p - ph) mod NX of the window at jx
+template <class R, int ORDER>
+__device__ __forceinline__ void flush_window(Acc<R, TWin<ORDER>::NX>& a, R* jx, int ph) {
+  using W = TWin<ORDER>;
+  constexpr int NX = W::NX;
+#pragma unroll
+  for (int p = 0; p < NX; ++p) {
+    int i = p - ph;
+    i += i < 0 ? NX : 0;
+    if (a.x[p] != R(0)) smem_add(jx + i, a.x[p]);
+    if (a.y[p] != R(0)) smem_add(jx + W::JVOL + i, a.y[p]);
+    if (a.z[p] != R(0)) smem_add(jx + 2 * W::JVOL + i, a.z[p]);
+  }
+  a.zero();
+}
+
 template <class R, int ORDER>
 __global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn,
                                                                      R* __restrict__ yn, R* __restrict__ zn,
@@ -181,12 +254,11 @@ __global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, 
                                                                      unsigned long long* deactivated) {
   using W = TWin<ORDER>;
   constexpr int NX = W::NX, NYZ = W::NYZ, LG = W::LG, EX = W::EX, EYZ = W::EYZ, JVOL = W::JVOL, REC = W::REC;
-  constexpr int GPW = 32 / LG;                       // groups per warp
-  constexpr int NGRP = kDepTileWarps * GPW;          // groups per CTA
+  constexpr int NG = 32 / LG;                        // groups per warp: particles in flight
   extern __shared__ __align__(16) unsigned char smem_raw[];
   R* Jt = reinterpret_cast<R*>(smem_raw);            // [3][EYZ][EYZ][EX]
   R* rec_all = Jt + 3 * JVOL + ((3 * JVOL) & 1);     // keep 16-byte alignment of the records
-  __shared__ int s_ib[kDepTileWarps][32];
+  __shared__ int s_code[kDepTileWarps][32];
 
   const int tile = blockIdx.x;
   const int s = tile_start[tile], e = tile_start[tile + 1];
@@ -199,48 +271,28 @@ __global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int grp = lane / LG, gl = lane % LG;
   const int j = gl % NYZ, k = gl / NYZ;
-  const int off_jk = EX * (j + EYZ * k);
+  R* const col = Jt + EX * (j + EYZ * k);            // this lane's (j,k) column of a window at box offset 0
   R* rec = rec_all + (size_t)warp * 32 * REC;
   const R half = R(0.5), third = R(1) / R(3);
 
+  // the warp's contiguous share of the tile, a multiple of 32 particles
   const int n = e - s;
-  const int chunk = ((n + NGRP - 1) / NGRP + LG - 1) / LG * LG;   // particles per group, multiple of LG
-  const int gb = s + (warp * GPW + grp) * chunk;
-  const int ge = min(e, gb + chunk);
-  const int rounds = chunk / LG;
+  const int chunk = ((n + kDepTileWarps - 1) / kDepTileWarps + 31) & ~31;
+  const int wb = s + warp * chunk;
+  const int we = min(e, wb + chunk);
 
-  R ax[NX - 1], ay[NX], az[NX];
-#pragma unroll
-  for (int i = 0; i < NX; ++i) { ay[i] = 0; az[i] = 0; if (i < NX - 1) ax[i] = 0; }
-  int cur = INT_MIN;   // J-box offset of the window base of the run being accumulated
+  Acc<R, NX> acc;
+  acc.zero();
+  int cur = INT_MIN;   // box offset of the window being accumulated (its first node), per group
+  int curph = 0;       // (x index of that node) mod NX
 
-  auto flush_all = [&]() {
-    if (cur == INT_MIN) return;
-    R* jx = Jt + cur + off_jk;
-#pragma unroll
-    for (int i = 0; i < NX; ++i) {
-      if (i < NX - 1 && ax[i] != R(0)) smem_add(jx + i, ax[i]);
-      if (ay[i] != R(0)) smem_add(jx + JVOL + i, ay[i]);
-      if (az[i] != R(0)) smem_add(jx + 2 * JVOL + i, az[i]);
-    }
-  };
-  auto shift_one = [&]() {   // the run moves one cell up in x: x-slot 0 is complete
-    R* jx = Jt + cur + off_jk;
-    if (ax[0] != R(0)) smem_add(jx, ax[0]);
-    if (ay[0] != R(0)) smem_add(jx + JVOL, ay[0]);
-    if (az[0] != R(0)) smem_add(jx + 2 * JVOL, az[0]);
-#pragma unroll
-    for (int i = 0; i < NX - 1; ++i) { ay[i] = ay[i + 1]; az[i] = az[i + 1]; if (i < NX - 2) ax[i] = ax[i + 1]; }
-    ay[NX - 1] = 0; az[NX - 1] = 0; ax[NX - 2] = 0;
-    cur += 1;
-  };
-
-  for (int r = 0; r < rounds; ++r) {
-    const int t = gb + r * LG + gl;
-    const bool valid = t < ge;
+  for (int rb = wb; rb < we; rb += 32) {
+    const int t = rb + lane;
+    const bool valid = t < we;
     bool elig = false;
     R x1[3] = {0, 0, 0};
     R w = 0;
+    int code = -1;
     if (valid) {
       R x0[3] = {p.x[t], p.y[t], p.z[t]};
       x1[0] = xn[t]; x1[1] = yn[t]; x1[2] = zn[t];
@@ -248,14 +300,14 @@ __global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, 
       R S0x[NX], DSx[NX], S0y[NYZ], DSy[NYZ], S0z[NYZ], DSz[NYZ];
       int c[3];
       bool fit[3];
-      axis_window<R, ORDER, NX, W::BLX>(x0[0] * g.inv_dx[0], x1[0] * g.inv_dx[0], g.N[0], c[0], S0x, DSx, fit[0]);
-      axis_window<R, ORDER, NYZ, W::BLYZ>(x0[1] * g.inv_dx[1], x1[1] * g.inv_dx[1], g.N[1], c[1], S0y, DSy, fit[1]);
-      axis_window<R, ORDER, NYZ, W::BLYZ>(x0[2] * g.inv_dx[2], x1[2] * g.inv_dx[2], g.N[2], c[2], S0z, DSz, fit[2]);
+      axis_window<R, ORDER, NX, W::BLX>(x0[0] * g.inv_dx[0], x1[0] * g.inv_dx[0], c[0], S0x, DSx, fit[0]);
+      axis_window<R, ORDER, NYZ, W::BLYZ>(x0[1] * g.inv_dx[1], x1[1] * g.inv_dx[1], c[1], S0y, DSy, fit[1]);
+      axis_window<R, ORDER, NYZ, W::BLYZ>(x0[2] * g.inv_dx[2], x1[2] * g.inv_dx[2], c[2], S0z, DSz, fit[2]);
       const int rc0 = c[0] - tb[0], rc1 = c[1] - tb[1], rc2 = c[2] - tb[2];
       elig = fit[0] & fit[1] & fit[2] & (rc0 >= 0) & (rc0 < ts.T[0]) & (rc1 >= 0) & (rc1 < ts.T[1]) & (rc2 >= 0) &
              (rc2 < ts.T[2]);
       if (elig) {
-        s_ib[warp][lane] = rc0 + EX * (rc1 + EYZ * rc2);
+        code = ((rc0 + EX * (rc1 + EYZ * rc2)) << 3) | (rc0 % NX);
         R* rr = rec + lane * REC;
         const R fx = -(w * p.jf[0]), fy = -(w * p.jf[1]), fz = -(w * p.jf[2]);
         R px = 0, py = 0, pz = 0;
@@ -276,39 +328,29 @@ __global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, 
         }
       }
     }
+    s_code[warp][lane] = code;
     __syncwarp();
-    const unsigned bal = __ballot_sync(0xffffffffu, elig);
-    const unsigned gm = (bal >> (grp * LG)) & (LG == 32 ? 0xffffffffu : ((1u << LG) - 1u));
+    // the NG groups take consecutive particles (mostly of one cell): q-th pass, particle q*NG + grp
 #pragma unroll 1
     for (int q = 0; q < LG; ++q) {
-      if (!((gm >> q) & 1u)) continue;
-      const int src = grp * LG + q;
-      const int ibq = s_ib[warp][src];
-      if (ibq != cur) {
-        const int sh = ibq - cur;
-        if (cur != INT_MIN && sh > 0 && sh < NX) {
-          for (int i = 0; i < sh; ++i) shift_one();
-        } else {
-          flush_all();
-#pragma unroll
-          for (int i = 0; i < NX; ++i) { ay[i] = 0; az[i] = 0; if (i < NX - 1) ax[i] = 0; }
-          cur = ibq;
-        }
-      }
+      const int src = q * NG + grp;
+      const int cd = s_code[warp][src];
+      if (cd < 0) continue;
+      const int ib = cd >> 3, ph = cd & 7;
+      const bool adv = ib == cur + 1;
+      R* const jx_old = col + cur;
+      if (ib != cur && !adv && cur != INT_MIN) flush_window<R, ORDER>(acc, jx_old, curph);
       const R* rr = rec + src * REC;
-      const Pair2<R> yv = *reinterpret_cast<const Pair2<R>*>(rr + W::oY + 2 * j);
-      const Pair2<R> zv = *reinterpret_cast<const Pair2<R>*>(rr + W::oZ + 2 * k);
-      const R py = rr[W::oPY + j], pz = rr[W::oPZ + k];
-      const R cx = zv.a * (yv.a + half * yv.b) + zv.b * (half * yv.a + third * yv.b);
-      const R q1 = py * zv.a, q2 = py * zv.b;
-      const R r1 = pz * yv.a, r2 = pz * yv.b;
-#pragma unroll
-      for (int i = 0; i < NX; ++i) {
-        const Pair2<R> ab = *reinterpret_cast<const Pair2<R>*>(rr + W::oAB + 2 * i);
-        if (i < NX - 1) ax[i] += cx * rr[W::oPX + i];
-        ay[i] += q1 * ab.a + q2 * ab.b;
-        az[i] += r1 * ab.a + r2 * ab.b;
+      switch (ph) {
+        case 0: step_phase<R, ORDER, 0>(acc, adv, jx_old, rr, j, k); break;
+        case 1: step_phase<R, ORDER, 1>(acc, adv, jx_old, rr, j, k); break;
+        case 2: step_phase<R, ORDER, 2>(acc, adv, jx_old, rr, j, k); break;
+        case 3: step_phase<R, ORDER, 3 % NX>(acc, adv, jx_old, rr, j, k); break;
+        case 4: step_phase<R, ORDER, 4 % NX>(acc, adv, jx_old, rr, j, k); break;
+        default: step_phase<R, ORDER, 5 % NX>(acc, adv, jx_old, rr, j, k); break;
       }
+      cur = ib;
+      curph = ph;
     }
     __syncwarp();
     // particles deposited here are finished: wrap and store; the others go to the list untouched
@@ -331,7 +373,7 @@ __global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, 
       xn[t] = x1[0]; yn[t] = x1[1]; zn[t] = x1[2];
     }
   }
-  flush_all();
+  if (cur != INT_MIN) flush_window<R, ORDER>(acc, col + cur, curph);
   __syncthreads();
   // the tile's J box -> global memory, one reduction per touched node
   const int b0 = tb[0] - W::BLX, b1 = tb[1] - W::BLYZ, b2 = tb[2] - W::BLYZ;
