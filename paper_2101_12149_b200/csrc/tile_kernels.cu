@@ -212,37 +212,57 @@ __device__ __forceinline__ void accumulate(Acc<R, TWin<ORDER>::NX>& a, const R* 
   }
 }
 
-// window advanced by one cell along x: the node that left (old logical slot 0, physical slot
-// PH - 1) goes to the box at jx_old[0]; then accumulate
-template <class R, int ORDER, int PH>
-__device__ __forceinline__ void step_phase(Acc<R, TWin<ORDER>::NX>& a, bool adv, R* jx_old, const R* __restrict__ rr,
-                                           int j, int k) {
-  using W = TWin<ORDER>;
-  constexpr int NX = W::NX;
-  constexpr int PO = (PH + NX - 1) % NX;
-  if (adv) {
-    if (a.x[PO] != R(0)) smem_add(jx_old, a.x[PO]);
-    if (a.y[PO] != R(0)) smem_add(jx_old + W::JVOL, a.y[PO]);
-    if (a.z[PO] != R(0)) smem_add(jx_old + 2 * W::JVOL, a.z[PO]);
-    a.x[PO] = 0; a.y[PO] = 0; a.z[PO] = 0;
-  }
-  accumulate<R, ORDER, PH>(a, rr, j, k);
+// sum over the NG groups of a warp (lanes that own the same column), result in every lane
+template <class R, int LG>
+__device__ __forceinline__ R group_sum(R v) {
+#pragma unroll
+  for (int o = LG; o < 32; o <<= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
 }
 
-// all slots to the box: physical slot p holds logical slot (p - ph) mod NX of the window at jx
+// one physical slot (static P) of all groups -> box element jx[0..2*JVOL], then cleared. Warp-uniform.
+template <class R, int ORDER, int P>
+__device__ __forceinline__ void flush_slot(Acc<R, TWin<ORDER>::NX>& a, R* jx, bool writer) {
+  using W = TWin<ORDER>;
+  const R vx = group_sum<R, W::LG>(a.x[P]), vy = group_sum<R, W::LG>(a.y[P]), vz = group_sum<R, W::LG>(a.z[P]);
+  if (writer) {
+    if (vx != R(0)) smem_add(jx, vx);
+    if (vy != R(0)) smem_add(jx + W::JVOL, vy);
+    if (vz != R(0)) smem_add(jx + 2 * W::JVOL, vz);
+  }
+  a.x[P] = 0; a.y[P] = 0; a.z[P] = 0;
+}
+
+// all slots: physical slot p holds logical slot (p - ph) mod NX of the window at jx. Warp-uniform.
 template <class R, int ORDER>
-__device__ __forceinline__ void flush_window(Acc<R, TWin<ORDER>::NX>& a, R* jx, int ph) {
+__device__ __forceinline__ void flush_window(Acc<R, TWin<ORDER>::NX>& a, R* jx, int ph, bool writer) {
   using W = TWin<ORDER>;
   constexpr int NX = W::NX;
 #pragma unroll
   for (int p = 0; p < NX; ++p) {
     int i = p - ph;
     i += i < 0 ? NX : 0;
-    if (a.x[p] != R(0)) smem_add(jx + i, a.x[p]);
-    if (a.y[p] != R(0)) smem_add(jx + W::JVOL + i, a.y[p]);
-    if (a.z[p] != R(0)) smem_add(jx + 2 * W::JVOL + i, a.z[p]);
+    const R vx = group_sum<R, W::LG>(a.x[p]), vy = group_sum<R, W::LG>(a.y[p]), vz = group_sum<R, W::LG>(a.z[p]);
+    if (writer) {
+      if (vx != R(0)) smem_add(jx + i, vx);
+      if (vy != R(0)) smem_add(jx + W::JVOL + i, vy);
+      if (vz != R(0)) smem_add(jx + 2 * W::JVOL + i, vz);
+    }
   }
   a.zero();
+}
+
+// the particles of one cell (cnt of them, record slots listed in order[]): NG at a time, one per
+// group. PH = (first box node of the cell's window) mod NX; adv = the window moved up one cell.
+template <class R, int ORDER, int PH>
+__device__ __forceinline__ void cell_batch(Acc<R, TWin<ORDER>::NX>& a, bool adv, R* jx_old, bool writer,
+                                           const R* __restrict__ rec, const int* __restrict__ order, int cnt, int grp,
+                                           int j, int k) {
+  using W = TWin<ORDER>;
+  constexpr int NX = W::NX, NG = 32 / W::LG;
+  if (adv) flush_slot<R, ORDER, (PH + NX - 1) % NX>(a, jx_old, writer);
+#pragma unroll 1
+  for (int it = grp; it < cnt; it += NG) accumulate<R, ORDER, PH>(a, rec + order[it] * W::REC, j, k);
 }
 
 template <class R, int ORDER>
@@ -254,11 +274,10 @@ __global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, 
                                                                      unsigned long long* deactivated) {
   using W = TWin<ORDER>;
   constexpr int NX = W::NX, NYZ = W::NYZ, LG = W::LG, EX = W::EX, EYZ = W::EYZ, JVOL = W::JVOL, REC = W::REC;
-  constexpr int NG = 32 / LG;                        // groups per warp: particles in flight
   extern __shared__ __align__(16) unsigned char smem_raw[];
   R* Jt = reinterpret_cast<R*>(smem_raw);            // [3][EYZ][EYZ][EX]
   R* rec_all = Jt + 3 * JVOL + ((3 * JVOL) & 1);     // keep 16-byte alignment of the records
-  __shared__ int s_code[kDepTileWarps][32];
+  __shared__ int s_order[kDepTileWarps][32];
 
   const int tile = blockIdx.x;
   const int s = tile_start[tile], e = tile_start[tile + 1];
@@ -328,31 +347,33 @@ __global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, 
         }
       }
     }
-    s_code[warp][lane] = code;
     __syncwarp();
-    // the NG groups take consecutive particles (mostly of one cell): q-th pass, particle q*NG + grp
-#pragma unroll 1
-    for (int q = 0; q < LG; ++q) {
-      const int src = q * NG + grp;
-      const int cd = s_code[warp][src];
-      if (cd < 0) continue;
+    // cell by cell (warp-uniform control flow): all particles of this round that share a window
+    unsigned rem = __ballot_sync(0xffffffffu, code >= 0);
+    while (rem) {
+      const int cd = __shfl_sync(0xffffffffu, code, __ffs(rem) - 1);
+      const unsigned m = __ballot_sync(0xffffffffu, code == cd);
+      rem &= ~m;
+      if ((m >> lane) & 1u) s_order[warp][__popc(m & ((1u << lane) - 1u))] = lane;
+      __syncwarp();
+      const int cnt = __popc(m);
       const int ib = cd >> 3, ph = cd & 7;
       const bool adv = ib == cur + 1;
       R* const jx_old = col + cur;
-      if (ib != cur && !adv && cur != INT_MIN) flush_window<R, ORDER>(acc, jx_old, curph);
-      const R* rr = rec + src * REC;
+      if (ib != cur && !adv && cur != INT_MIN) flush_window<R, ORDER>(acc, jx_old, curph, grp == 0);
+      const int* ord = s_order[warp];
       switch (ph) {
-        case 0: step_phase<R, ORDER, 0>(acc, adv, jx_old, rr, j, k); break;
-        case 1: step_phase<R, ORDER, 1>(acc, adv, jx_old, rr, j, k); break;
-        case 2: step_phase<R, ORDER, 2>(acc, adv, jx_old, rr, j, k); break;
-        case 3: step_phase<R, ORDER, 3 % NX>(acc, adv, jx_old, rr, j, k); break;
-        case 4: step_phase<R, ORDER, 4 % NX>(acc, adv, jx_old, rr, j, k); break;
-        default: step_phase<R, ORDER, 5 % NX>(acc, adv, jx_old, rr, j, k); break;
+        case 0: cell_batch<R, ORDER, 0>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 1: cell_batch<R, ORDER, 1>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 2: cell_batch<R, ORDER, 2>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 3: cell_batch<R, ORDER, 3 % NX>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 4: cell_batch<R, ORDER, 4 % NX>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        default: cell_batch<R, ORDER, 5 % NX>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
       }
       cur = ib;
       curph = ph;
+      __syncwarp();
     }
-    __syncwarp();
     // particles deposited here are finished: wrap and store; the others go to the list untouched
     const bool stray = valid && !elig;
     const unsigned sm = __ballot_sync(0xffffffffu, stray);
@@ -373,7 +394,7 @@ __global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, 
       xn[t] = x1[0]; yn[t] = x1[1]; zn[t] = x1[2];
     }
   }
-  if (cur != INT_MIN) flush_window<R, ORDER>(acc, col + cur, curph);
+  if (cur != INT_MIN) flush_window<R, ORDER>(acc, col + cur, curph, grp == 0);
   __syncthreads();
   // the tile's J box -> global memory, one reduction per touched node
   const int b0 = tb[0] - W::BLX, b1 = tb[1] - W::BLYZ, b2 = tb[2] - W::BLYZ;
