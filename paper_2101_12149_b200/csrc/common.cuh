@@ -78,6 +78,11 @@ __device__ __forceinline__ int shape(R xi, R* w) {
 __device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
 __device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
 
+// difference of two ROUNDED values: keeps the compiler from contracting the last multiply of a
+// shape weight into the subtraction (DS = S1 - S0 cancels to roundoff for a slow particle)
+__device__ __forceinline__ double sub_rn(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ float sub_rn(float a, float b) { return __fsub_rn(a, b); }
+
 template <class R>
 __device__ __forceinline__ int cell_of(R x, R inv_dx, int N) {
   int c = (int)floor(mul_rn(x, inv_dx));

@@ -10,7 +10,9 @@
 //                   into the tile's J box in shared memory, and reach global memory once per tile.
 // Particles that no longer fit the tile's boxes (they drifted since the last sort) are handled by
 // the global-memory paths in particles.cu; correctness never depends on the order or the tile.
+#include <algorithm>
 #include <climits>
+#include <cstdlib>
 
 #include "internal.h"
 #include "particle_math.cuh"
@@ -158,6 +160,30 @@ __device__ __forceinline__ void axis_window(R xi0, R xi1, int& cell, R* S0, R* D
   const int l0 = shape<R, ORDER>(xi0, w0);
   const int l1 = shape<R, ORDER>(xi1, w1);
   const int c = ORDER == 2 ? (int)floor(xi0) : (ORDER == 1 ? l0 : l0 + 1);
+  cell = c;
+  if constexpr (ORDER != 2 && NW == ORDER + 1) {
+    // tight window: it is the old support itself; the new one fits only if it starts at the same node
+#pragma unroll
+    for (int i = 0; i < NW; ++i) { S0[i] = w0[i]; DS[i] = sub_rn(w1[i], w0[i]); }
+    fits = l1 == l0;
+    return;
+  } else if constexpr (ORDER != 2 && NW == ORDER + 3) {
+    // old support at slots 1..ORDER+1; the new one starts at slot 0, 1 or 2
+    const int sl1 = l1 - l0 + 1;
+    const bool d0 = sl1 == 0, d2 = sl1 == 2;
+#pragma unroll
+    for (int i = 0; i < NW; ++i) {
+      const R lo = i <= ORDER ? w1[i <= ORDER ? i : 0] : R(0);
+      const R mid = (i >= 1 && i <= ORDER + 1) ? w1[(i >= 1 && i <= ORDER + 1) ? i - 1 : 0] : R(0);
+      const R hi = i >= 2 ? w1[i >= 2 ? i - 2 : 0] : R(0);
+      const R a = (i >= 1 && i <= ORDER + 1) ? w0[(i >= 1 && i <= ORDER + 1) ? i - 1 : 0] : R(0);
+      const R b = d0 ? lo : (d2 ? hi : mid);
+      S0[i] = a;
+      DS[i] = sub_rn(b, a);
+    }
+    fits = (sl1 >= 0) & (sl1 <= 2);
+    return;
+  }
   const int so0 = ORDER == 2 ? l0 - (c - BL) : (ORDER == 1 ? BL : BL - 1);
   const int sl1 = l1 - (c - BL);
 #pragma unroll
@@ -172,7 +198,6 @@ __device__ __forceinline__ void axis_window(R xi0, R xi1, int& cell, R* S0, R* D
     DS[i] = b - a;
   }
   fits = (so0 >= 0) & (so0 + ORDER < NW) & (sl1 >= 0) & (sl1 + ORDER < NW);
-  cell = c;
 }
 
 __device__ __forceinline__ void smem_add(double* p, double v) { atomicAdd(p, v); }   // CAS loop on sm_100a
@@ -212,6 +237,15 @@ __device__ __forceinline__ void accumulate(Acc<R, TWin<ORDER>::NX>& a, const R* 
   }
 }
 
+// where a window's first node lives, per component: the tile's J box in shared memory, or (GLOBAL)
+// the J arrays themselves
+template <class R>
+struct JPtr { R* p[3]; };
+template <bool GLOBAL, class R>
+__device__ __forceinline__ void j_add(R* p, R v) {
+  if constexpr (GLOBAL) red_add(p, v); else smem_add(p, v);
+}
+
 // sum over the NG groups of a warp (lanes that own the same column), result in every lane
 template <class R, int LG>
 __device__ __forceinline__ R group_sum(R v) {
@@ -221,21 +255,21 @@ __device__ __forceinline__ R group_sum(R v) {
 }
 
 // one physical slot (static P) of all groups -> box element jx[0..2*JVOL], then cleared. Warp-uniform.
-template <class R, int ORDER, int P>
-__device__ __forceinline__ void flush_slot(Acc<R, TWin<ORDER>::NX>& a, R* jx, bool writer) {
+template <class R, int ORDER, int P, bool GLOBAL>
+__device__ __forceinline__ void flush_slot(Acc<R, TWin<ORDER>::NX>& a, const JPtr<R>& jx, bool writer) {
   using W = TWin<ORDER>;
   const R vx = group_sum<R, W::LG>(a.x[P]), vy = group_sum<R, W::LG>(a.y[P]), vz = group_sum<R, W::LG>(a.z[P]);
   if (writer) {
-    if (vx != R(0)) smem_add(jx, vx);
-    if (vy != R(0)) smem_add(jx + W::JVOL, vy);
-    if (vz != R(0)) smem_add(jx + 2 * W::JVOL, vz);
+    if (vx != R(0)) j_add<GLOBAL>(jx.p[0], vx);
+    if (vy != R(0)) j_add<GLOBAL>(jx.p[1], vy);
+    if (vz != R(0)) j_add<GLOBAL>(jx.p[2], vz);
   }
   a.x[P] = 0; a.y[P] = 0; a.z[P] = 0;
 }
 
 // all slots: physical slot p holds logical slot (p - ph) mod NX of the window at jx. Warp-uniform.
-template <class R, int ORDER>
-__device__ __forceinline__ void flush_window(Acc<R, TWin<ORDER>::NX>& a, R* jx, int ph, bool writer) {
+template <class R, int ORDER, bool GLOBAL>
+__device__ __forceinline__ void flush_window(Acc<R, TWin<ORDER>::NX>& a, const JPtr<R>& jx, int ph, bool writer) {
   using W = TWin<ORDER>;
   constexpr int NX = W::NX;
 #pragma unroll
@@ -244,9 +278,9 @@ __device__ __forceinline__ void flush_window(Acc<R, TWin<ORDER>::NX>& a, R* jx, 
     i += i < 0 ? NX : 0;
     const R vx = group_sum<R, W::LG>(a.x[p]), vy = group_sum<R, W::LG>(a.y[p]), vz = group_sum<R, W::LG>(a.z[p]);
     if (writer) {
-      if (vx != R(0)) smem_add(jx + i, vx);
-      if (vy != R(0)) smem_add(jx + W::JVOL + i, vy);
-      if (vz != R(0)) smem_add(jx + 2 * W::JVOL + i, vz);
+      if (vx != R(0)) j_add<GLOBAL>(jx.p[0] + i, vx);
+      if (vy != R(0)) j_add<GLOBAL>(jx.p[1] + i, vy);
+      if (vz != R(0)) j_add<GLOBAL>(jx.p[2] + i, vz);
     }
   }
   a.zero();
@@ -254,49 +288,65 @@ __device__ __forceinline__ void flush_window(Acc<R, TWin<ORDER>::NX>& a, R* jx, 
 
 // the particles of one cell (cnt of them, record slots listed in order[]): NG at a time, one per
 // group. PH = (first box node of the cell's window) mod NX; adv = the window moved up one cell.
-template <class R, int ORDER, int PH>
-__device__ __forceinline__ void cell_batch(Acc<R, TWin<ORDER>::NX>& a, bool adv, R* jx_old, bool writer,
+template <class R, int ORDER, int PH, bool GLOBAL>
+__device__ __forceinline__ void cell_batch(Acc<R, TWin<ORDER>::NX>& a, bool adv, const JPtr<R>& jx_old, bool writer,
                                            const R* __restrict__ rec, const int* __restrict__ order, int cnt, int grp,
                                            int j, int k) {
   using W = TWin<ORDER>;
   constexpr int NX = W::NX, NG = 32 / W::LG;
-  if (adv) flush_slot<R, ORDER, (PH + NX - 1) % NX>(a, jx_old, writer);
+  if (adv) flush_slot<R, ORDER, (PH + NX - 1) % NX, GLOBAL>(a, jx_old, writer);
 #pragma unroll 1
   for (int it = grp; it < cnt; it += NG) accumulate<R, ORDER, PH>(a, rec + order[it] * W::REC, j, k);
 }
 
-template <class R, int ORDER>
-__global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn,
-                                                                     R* __restrict__ yn, R* __restrict__ zn,
-                                                                     const int32_t* __restrict__ tile_start, TileSpec ts,
-                                                                     int32_t* __restrict__ stray_list,
-                                                                     unsigned int* __restrict__ stray_count,
-                                                                     unsigned long long* deactivated) {
+// GLOBAL = false: sums go to the tile's J box in shared memory and reach the J arrays once per tile;
+// GLOBAL = true: no box, every finished window node is one reduction at L2 (smaller CTAs, no
+// prologue/epilogue, no block barrier).
+template <class R, int ORDER, bool GLOBAL, int NWARP>
+__global__ void __launch_bounds__(NWARP * 32, GLOBAL ? 2 : 1)
+    k_deposit_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn, R* __restrict__ yn, R* __restrict__ zn,
+                   const int32_t* __restrict__ tile_start, TileSpec ts, int32_t* __restrict__ stray_list,
+                   unsigned int* __restrict__ stray_count, unsigned long long* deactivated) {
   using W = TWin<ORDER>;
   constexpr int NX = W::NX, NYZ = W::NYZ, LG = W::LG, EX = W::EX, EYZ = W::EYZ, JVOL = W::JVOL, REC = W::REC;
+  constexpr int JBOX = GLOBAL ? 0 : 3 * JVOL + ((3 * JVOL) & 1);   // keeps the records 16-byte aligned
   extern __shared__ __align__(16) unsigned char smem_raw[];
   R* Jt = reinterpret_cast<R*>(smem_raw);            // [3][EYZ][EYZ][EX]
-  R* rec_all = Jt + 3 * JVOL + ((3 * JVOL) & 1);     // keep 16-byte alignment of the records
-  __shared__ int s_order[kDepTileWarps][32];
+  R* rec_all = Jt + JBOX;
+  __shared__ int s_order[NWARP][32];
 
   const int tile = blockIdx.x;
   const int s = tile_start[tile], e = tile_start[tile + 1];
   if (s >= e) return;
   int tb[3];
   tile_coords(ts, tile, tb);
-  for (int i = threadIdx.x; i < 3 * JVOL; i += blockDim.x) Jt[i] = R(0);
-  __syncthreads();
+  if constexpr (!GLOBAL) {
+    for (int i = threadIdx.x; i < 3 * JVOL; i += blockDim.x) Jt[i] = R(0);
+    __syncthreads();
+  }
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int grp = lane / LG, gl = lane % LG;
   const int j = gl % NYZ, k = gl / NYZ;
-  R* const col = Jt + EX * (j + EYZ * k);            // this lane's (j,k) column of a window at box offset 0
+  // first node of this lane's (j,k) column of the window whose box offset is `off`
+  const int b0 = tb[0] - W::BLX, b1 = tb[1] - W::BLYZ, b2 = tb[2] - W::BLYZ;
+  auto column = [&](int off) {
+    JPtr<R> q;
+    if constexpr (GLOBAL) {
+      const int gi = g.idx(b0 + (off & 15), b1 + ((off >> 4) & 15) + j, b2 + (off >> 8) + k);
+      q.p[0] = g.J[0] + gi; q.p[1] = g.J[1] + gi; q.p[2] = g.J[2] + gi;
+    } else {
+      R* c0 = Jt + (off & 15) + EX * (((off >> 4) & 15) + j + EYZ * ((off >> 8) + k));
+      q.p[0] = c0; q.p[1] = c0 + JVOL; q.p[2] = c0 + 2 * JVOL;
+    }
+    return q;
+  };
   R* rec = rec_all + (size_t)warp * 32 * REC;
   const R half = R(0.5), third = R(1) / R(3);
 
   // the warp's contiguous share of the tile, a multiple of 32 particles
   const int n = e - s;
-  const int chunk = ((n + kDepTileWarps - 1) / kDepTileWarps + 31) & ~31;
+  const int chunk = ((n + NWARP - 1) / NWARP + 31) & ~31;
   const int wb = s + warp * chunk;
   const int we = min(e, wb + chunk);
 
@@ -326,7 +376,7 @@ __global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, 
       elig = fit[0] & fit[1] & fit[2] & (rc0 >= 0) & (rc0 < ts.T[0]) & (rc1 >= 0) & (rc1 < ts.T[1]) & (rc2 >= 0) &
              (rc2 < ts.T[2]);
       if (elig) {
-        code = ((rc0 + EX * (rc1 + EYZ * rc2)) << 3) | (rc0 % NX);
+        code = ((rc0 | (rc1 << 4) | (rc2 << 8)) << 3) | (rc0 % NX);
         R* rr = rec + lane * REC;
         const R fx = -(w * p.jf[0]), fy = -(w * p.jf[1]), fz = -(w * p.jf[2]);
         R px = 0, py = 0, pz = 0;
@@ -359,16 +409,17 @@ __global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, 
       const int cnt = __popc(m);
       const int ib = cd >> 3, ph = cd & 7;
       const bool adv = ib == cur + 1;
-      R* const jx_old = col + cur;
-      if (ib != cur && !adv && cur != INT_MIN) flush_window<R, ORDER>(acc, jx_old, curph, grp == 0);
+      JPtr<R> jx_old{};
+      if (cur != INT_MIN) jx_old = column(cur);
+      if (ib != cur && !adv && cur != INT_MIN) flush_window<R, ORDER, GLOBAL>(acc, jx_old, curph, grp == 0);
       const int* ord = s_order[warp];
       switch (ph) {
-        case 0: cell_batch<R, ORDER, 0>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 1: cell_batch<R, ORDER, 1>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 2: cell_batch<R, ORDER, 2>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 3: cell_batch<R, ORDER, 3 % NX>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 4: cell_batch<R, ORDER, 4 % NX>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        default: cell_batch<R, ORDER, 5 % NX>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 0: cell_batch<R, ORDER, 0, GLOBAL>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 1: cell_batch<R, ORDER, 1, GLOBAL>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 2: cell_batch<R, ORDER, 2, GLOBAL>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 3: cell_batch<R, ORDER, 3 % NX, GLOBAL>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 4: cell_batch<R, ORDER, 4 % NX, GLOBAL>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        default: cell_batch<R, ORDER, 5 % NX, GLOBAL>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
       }
       cur = ib;
       curph = ph;
@@ -394,10 +445,10 @@ __global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, 
       xn[t] = x1[0]; yn[t] = x1[1]; zn[t] = x1[2];
     }
   }
-  if (cur != INT_MIN) flush_window<R, ORDER>(acc, col + cur, curph, grp == 0);
+  if (cur != INT_MIN) flush_window<R, ORDER, GLOBAL>(acc, column(cur), curph, grp == 0);
+  if constexpr (GLOBAL) return;
   __syncthreads();
   // the tile's J box -> global memory, one reduction per touched node
-  const int b0 = tb[0] - W::BLX, b1 = tb[1] - W::BLYZ, b2 = tb[2] - W::BLYZ;
   for (int idx = threadIdx.x; idx < JVOL; idx += blockDim.x) {
     const int i = idx % EX, rr = idx / EX;
     const int jj = rr % EYZ, kk = rr / EYZ;
@@ -413,9 +464,10 @@ __global__ void __launch_bounds__(kDepTileWarps * 32) k_deposit_tile(Grid<R> g, 
 }  // namespace
 
 template <int ORDER, class R>
-static size_t dep_smem_bytes() {
+static size_t dep_smem_bytes(bool global, int nwarp) {
   using W = TWin<ORDER>;
-  return (size_t)(3 * W::JVOL + ((3 * W::JVOL) & 1) + kDepTileWarps * 32 * W::REC) * sizeof(R);
+  const size_t jbox = global ? 0 : 3 * W::JVOL + ((3 * W::JVOL) & 1);
+  return (jbox + (size_t)nwarp * 32 * W::REC) * sizeof(R);
 }
 
 template <class R, int ORDER>
@@ -424,11 +476,18 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, Ctx& c
   R *xn = a.alt.x, *yn = a.alt.y, *zn = a.alt.z;
   const int n_tiles = a.tiles.nt[0] * a.tiles.nt[1] * a.tiles.nt[2];
   static bool attr_set = false;
+  static int variant = 1;
   const size_t push_smem = (size_t)6 * PushBox<ORDER>::VOL * sizeof(R);
-  const size_t dep_smem = dep_smem_bytes<ORDER, R>();
+  constexpr int kGW = 8;
+  auto kbox = k_deposit_tile<R, ORDER, false, kDepTileWarps>;
+  auto kglb = k_deposit_tile<R, ORDER, true, kGW>;
+  const size_t box_smem = dep_smem_bytes<ORDER, R>(false, kDepTileWarps);
+  const size_t glb_smem = dep_smem_bytes<ORDER, R>(true, kGW);
   if (!attr_set) {
+    if (const char* v = getenv("PIC_DEP_VARIANT")) variant = atoi(v);
     cudaFuncSetAttribute(k_push_tile<R, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
-    cudaFuncSetAttribute(k_deposit_tile<R, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dep_smem);
+    cudaFuncSetAttribute(kbox, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)box_smem);
+    cudaFuncSetAttribute(kglb, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)glb_smem);
     attr_set = true;
   }
   {
@@ -437,8 +496,12 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, Ctx& c
   }
   {
     ScopedPhase ph(c, kPhaseDeposit);
-    k_deposit_tile<R, ORDER><<<n_tiles, kDepTileWarps * 32, dep_smem, c.stream>>>(
-        g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list, a.stray_count, a.deactivated);
+    if (variant == 1)
+      kglb<<<n_tiles, kGW * 32, glb_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
+                                                     a.stray_count, a.deactivated);
+    else
+      kbox<<<n_tiles, kDepTileWarps * 32, box_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
+                                                               a.stray_count, a.deactivated);
   }
   c.launches += 2;
 }
