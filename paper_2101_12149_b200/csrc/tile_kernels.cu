@@ -461,6 +461,242 @@ __global__ void __launch_bounds__(NWARP * 32, GLOBAL ? 2 : 1)
   }
 }
 
+// =================================================================== Esirkepov on the fp64 tensor pipe
+// The sums of one cell's particles are small dense contractions over the particles p:
+//   Jx[i][jk] += sum_p PX_p[i] * cx_p[jk]
+//   Jy[i][jk] += sum_p A_p[i] * (PY_p[j] S0z_p[k]) + B_p[i] * (PY_p[j] DSz_p[k])       (Jz alike)
+// with i the NX window nodes along x and jk the NYZ^2 columns, i.e. C[8 x 16] += A[8 x K] B[K x 16],
+// K = particles (Jx) or 2 x particles (Jy, Jz): mma.sync.m8n8k4.f64 (DMMA), one warp per cell batch.
+// Row r of C holds window node X with X mod 8 == r, so C never moves when the window advances: the
+// row of the node that left is reduced into J (one RED per element) and reused.
+__device__ __forceinline__ void dmma_884(double& c0, double& c1, double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(c0), "+d"(c1)
+               : "d"(a), "d"(b));
+}
+
+template <int ORDER>
+struct MWin {
+  using T = TWin<ORDER>;
+  static constexpr int NX = T::NX, BLX = T::BLX, NYZ = T::NYZ, BLYZ = T::BLYZ;
+  static constexpr int NCOL = NYZ * NYZ;              // 16 (orders 2, 3) or 4 (order 1)
+  static constexpr int NB = NCOL > 8 ? NCOL / 8 : 1;  // 8-column blocks of C
+  static constexpr int KSTEP = NYZ == 4 ? 2 : 0;      // k advances by this from one column block to the next
+  // record (elements): {A_x,B_x}[NX] | PX[NX] | {al_y,be_y}[NYZ] | {S0_y,DS_y}[NYZ] | PY[NYZ] |
+  //                    {S0_z,DS_z}[NYZ] | PZ[NYZ]
+  static constexpr int oAB = 0, oPX = 2 * NX, oYab = 3 * NX, oY = oYab + 2 * NYZ, oPY = oY + 2 * NYZ,
+                       oZ = oPY + NYZ, oPZ = oZ + 2 * NYZ;
+  static constexpr int RAW = oPZ + NYZ;                            // 50 / 28
+  static constexpr int REC = (RAW / 2) % 2 == 1 ? RAW : RAW + 2;   // REC/2 odd: conflict-free pair stores
+};
+
+// C fragments of one lane: rows = window nodes (lane >> 2), columns 2*(lane & 3) + {0,1} of each block
+template <int NB>
+struct CFrag {
+  double x[NB][2], y[NB][2], z[NB][2];
+  __device__ __forceinline__ void zero() {
+#pragma unroll
+    for (int b = 0; b < NB; ++b)
+#pragma unroll
+      for (int e = 0; e < 2; ++e) { x[b][e] = 0; y[b][e] = 0; z[b][e] = 0; }
+  }
+};
+
+template <class R, int ORDER, int NWARP>
+__global__ void __launch_bounds__(NWARP * 32, 2)
+    k_deposit_mma(Grid<R> g, Particles<R> p, R* __restrict__ xn, R* __restrict__ yn, R* __restrict__ zn,
+                  const int32_t* __restrict__ tile_start, TileSpec ts, int32_t* __restrict__ stray_list,
+                  unsigned int* __restrict__ stray_count, unsigned long long* deactivated) {
+  using W = MWin<ORDER>;
+  constexpr int NX = W::NX, NYZ = W::NYZ, NB = W::NB, REC = W::REC, BLX = W::BLX, BLYZ = W::BLYZ;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  R* rec_all = reinterpret_cast<R*>(smem_raw);
+
+  const int tile = blockIdx.x;
+  const int s = tile_start[tile], e = tile_start[tile + 1];
+  if (s >= e) return;
+  int tb[3];
+  tile_coords(ts, tile, tb);
+
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int gq = lane >> 2, t = lane & 3;           // fragment coordinates of this lane
+  const int term = t & 1;
+  R* rec = rec_all + (size_t)warp * 33 * REC;       // 32 records of the round + one that stays zero
+  const R* zrec = rec + 32 * REC;
+  for (int i = lane; i < REC; i += 32) rec[32 * REC + i] = R(0);
+  const R half = R(0.5), third = R(1) / R(3);
+
+  // B operands: this lane supplies column gq (+ 8 per block) = (jB, kB + KSTEP * block)
+  const bool colok = gq < W::NCOL;
+  const int jB = colok ? gq % NYZ : 0, kB = colok ? gq / NYZ : 0;
+  const int offYab = W::oYab + 2 * jB, offY = W::oY + 2 * jB, offPY = W::oPY + jB, offZ = W::oZ + 2 * kB,
+            offPZ = W::oPZ + kB;
+  // C fragments: this lane holds columns 2t + {0,1} (+ 8 per block) of row gq
+  int coff[NB][2];
+  bool cok[NB][2];
+#pragma unroll
+  for (int b = 0; b < NB; ++b)
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      const int n = 2 * t + c + 8 * b;
+      cok[b][c] = n < W::NCOL;
+      coff[b][c] = (n % NYZ) * g.sy + (n / NYZ) * g.sz;
+    }
+
+  CFrag<NB> C;
+  C.zero();
+  int cur = INT_MIN;   // packed cell of the window being accumulated
+  auto win_x = [&](int cd) { return tb[0] + (cd & 15) - 4 - BLX; };
+  auto win_y = [&](int cd) { return tb[1] + ((cd >> 4) & 15) - 4 - BLYZ; };
+  auto win_z = [&](int cd) { return tb[2] + (cd >> 8) - 4 - BLYZ; };
+  // rows of the old window that the new one (nx0 .. nx0+NX-1 on the same y,z; none if !same_row) does
+  // not contain go to J, one reduction per element, and are cleared
+  auto retire_rows = [&](bool same_row, int nx0) {
+    const int ox0 = win_x(cur);
+    const int io = (gq - ox0) & 7;
+    const int X = ox0 + io;
+    const bool keep = same_row && X >= nx0 && X < nx0 + NX;
+    if (io < NX && !keep) {
+      const int base = g.idx(X, win_y(cur), win_z(cur));
+#pragma unroll
+      for (int b = 0; b < NB; ++b)
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+          if (cok[b][c]) {
+            if (C.x[b][c] != 0.0) red_add(g.J[0] + base + coff[b][c], (R)C.x[b][c]);
+            if (C.y[b][c] != 0.0) red_add(g.J[1] + base + coff[b][c], (R)C.y[b][c]);
+            if (C.z[b][c] != 0.0) red_add(g.J[2] + base + coff[b][c], (R)C.z[b][c]);
+          }
+          C.x[b][c] = 0; C.y[b][c] = 0; C.z[b][c] = 0;
+        }
+    }
+  };
+
+  // the warp's contiguous share of the tile, a multiple of 32 particles
+  const int n = e - s;
+  const int chunk = ((n + NWARP - 1) / NWARP + 31) & ~31;
+  const int wb = s + warp * chunk;
+  const int we = min(e, wb + chunk);
+
+  for (int rb = wb; rb < we; rb += 32) {
+    const int tp = rb + lane;
+    const bool valid = tp < we;
+    bool elig = false;
+    R x1[3] = {0, 0, 0};
+    R w = 0;
+    int code = -1;
+    if (valid) {
+      R x0[3] = {p.x[tp], p.y[tp], p.z[tp]};
+      x1[0] = xn[tp]; x1[1] = yn[tp]; x1[2] = zn[tp];
+      w = p.w[tp];
+      R S0x[NX], DSx[NX], S0y[NYZ], DSy[NYZ], S0z[NYZ], DSz[NYZ];
+      int c[3];
+      bool fit[3];
+      axis_window<R, ORDER, NX, BLX>(x0[0] * g.inv_dx[0], x1[0] * g.inv_dx[0], c[0], S0x, DSx, fit[0]);
+      axis_window<R, ORDER, NYZ, BLYZ>(x0[1] * g.inv_dx[1], x1[1] * g.inv_dx[1], c[1], S0y, DSy, fit[1]);
+      axis_window<R, ORDER, NYZ, BLYZ>(x0[2] * g.inv_dx[2], x1[2] * g.inv_dx[2], c[2], S0z, DSz, fit[2]);
+      // the cell must be inside the grid and within 4 cells of the tile (4-bit biased offsets)
+      const int rc0 = c[0] - tb[0] + 4, rc1 = c[1] - tb[1] + 4, rc2 = c[2] - tb[2] + 4;
+      elig = fit[0] & fit[1] & fit[2] & (((rc0 | rc1 | rc2) & ~15) == 0) & (c[0] >= 0) & (c[0] < g.N[0]) &
+             (c[1] >= 0) & (c[1] < g.N[1]) & (c[2] >= 0) & (c[2] < g.N[2]);
+      if (elig) {
+        code = rc0 | (rc1 << 4) | (rc2 << 8);
+        R* rr = rec + lane * REC;
+        const R fx = -(w * p.jf[0]), fy = -(w * p.jf[1]), fz = -(w * p.jf[2]);
+        R px = 0, py = 0, pz = 0;
+#pragma unroll
+        for (int i = 0; i < NX; ++i) {
+          *reinterpret_cast<Pair2<R>*>(rr + W::oAB + 2 * i) =
+              Pair2<R>{S0x[i] + half * DSx[i], half * S0x[i] + third * DSx[i]};
+          px += DSx[i];
+          rr[W::oPX + i] = fx * px;
+        }
+#pragma unroll
+        for (int i = 0; i < NYZ; ++i) {
+          *reinterpret_cast<Pair2<R>*>(rr + W::oYab + 2 * i) =
+              Pair2<R>{S0y[i] + half * DSy[i], half * S0y[i] + third * DSy[i]};
+          *reinterpret_cast<Pair2<R>*>(rr + W::oY + 2 * i) = Pair2<R>{S0y[i], DSy[i]};
+          *reinterpret_cast<Pair2<R>*>(rr + W::oZ + 2 * i) = Pair2<R>{S0z[i], DSz[i]};
+          py += DSy[i]; pz += DSz[i];
+          rr[W::oPY + i] = fy * py;
+          rr[W::oPZ + i] = fz * pz;
+        }
+      }
+    }
+    __syncwarp();
+    // runs of consecutive particles with the same window (the order is cell-sorted up to drift since
+    // the last sort; a cell met twice is simply accumulated twice). Warp-uniform control flow.
+    const int prev = __shfl_up_sync(0xffffffffu, code, 1);
+    unsigned heads = __ballot_sync(0xffffffffu, lane == 0 || code != prev);
+    const unsigned live = __ballot_sync(0xffffffffu, code >= 0);
+    while (heads) {
+      const int s0 = __ffs(heads) - 1;
+      heads &= heads - 1;
+      const int s1 = heads ? __ffs(heads) - 1 : 32;
+      if (!((live >> s0) & 1u)) continue;
+      const int cd = __shfl_sync(0xffffffffu, code, s0);
+      if (cd != cur) {
+        if (cur != INT_MIN) retire_rows(((cd ^ cur) >> 4) == 0, win_x(cd));
+        cur = cd;
+      }
+      const int i = (gq - win_x(cd)) & 7;          // window slot of this lane's row
+      const bool rowok = i < NX;
+      const int offPX = W::oPX + (rowok ? i : 0), offAB = W::oAB + 2 * (rowok ? i : 0) + term;
+#pragma unroll 2
+      for (int b = s0; b < s1; b += 4) {
+        {   // Jx: four particles, K = particle
+          const R* rr = rec + (b + t < s1 ? b + t : 32) * REC;      // slot 32: the all-zero record
+          const R* ra = rowok ? rr : zrec;
+          const double a = ra[offPX];
+          const Pair2<R> ab = *reinterpret_cast<const Pair2<R>*>(rr + offYab);
+#pragma unroll
+          for (int nb = 0; nb < NB; ++nb) {
+            const Pair2<R> zv = *reinterpret_cast<const Pair2<R>*>(rr + offZ + 2 * W::KSTEP * nb);
+            const double cx = fma((double)zv.a, (double)ab.a, (double)zv.b * (double)ab.b);
+            dmma_884(C.x[nb][0], C.x[nb][1], a, colok ? cx : 0.0);
+          }
+        }
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {   // Jy, Jz: two particles each, K = (particle, term)
+          if (q == 1 && b + 2 >= s1) break;
+          const int idx = b + 2 * q + (t >> 1);
+          const R* rr = rec + (idx < s1 ? idx : 32) * REC;
+          const R* ra = rowok ? rr : zrec;
+          const double a = ra[offAB];
+          const double yel = rr[offY + term], py = rr[offPY];
+#pragma unroll
+          for (int nb = 0; nb < NB; ++nb) {
+            const double zel = rr[offZ + 2 * W::KSTEP * nb + term], pz = rr[offPZ + W::KSTEP * nb];
+            dmma_884(C.y[nb][0], C.y[nb][1], a, colok ? py * zel : 0.0);
+            dmma_884(C.z[nb][0], C.z[nb][1], a, colok ? pz * yel : 0.0);
+          }
+        }
+      }
+    }
+    __syncwarp();
+    // particles deposited here are finished: wrap and store; the others go to the list untouched
+    const bool stray = valid && !elig;
+    const unsigned sm = __ballot_sync(0xffffffffu, stray);
+    if (sm) {
+      unsigned base = 0;
+      if (lane == 0) base = atomicAdd(stray_count, (unsigned)__popc(sm));
+      base = __shfl_sync(0xffffffffu, base, 0);
+      if (stray) stray_list[base + __popc(sm & ((1u << lane) - 1u))] = (int32_t)tp;
+    }
+    if (valid && elig) {
+      bool out = false;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) out |= wrap_axis<R>(x1[d], g.L[d], g.periodic[d]);
+      if (out) {
+        if (w != R(0)) atomicAdd(deactivated, 1ull);
+        p.w[tp] = R(0);
+      }
+      xn[tp] = x1[0]; yn[tp] = x1[1]; zn[tp] = x1[2];
+    }
+  }
+  if (cur != INT_MIN) retire_rows(false, 0);
+}
+
 }  // namespace
 
 template <int ORDER, class R>
@@ -476,11 +712,13 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, Ctx& c
   R *xn = a.alt.x, *yn = a.alt.y, *zn = a.alt.z;
   const int n_tiles = a.tiles.nt[0] * a.tiles.nt[1] * a.tiles.nt[2];
   static bool attr_set = false;
-  static int variant = 1;
+  static int variant = 2;
   const size_t push_smem = (size_t)6 * PushBox<ORDER>::VOL * sizeof(R);
   constexpr int kGW = 8;
   auto kbox = k_deposit_tile<R, ORDER, false, kDepTileWarps>;
   auto kglb = k_deposit_tile<R, ORDER, true, kGW>;
+  auto kmma = k_deposit_mma<R, ORDER, kGW>;
+  const size_t mma_smem = (size_t)kGW * 33 * MWin<ORDER>::REC * sizeof(R);
   const size_t box_smem = dep_smem_bytes<ORDER, R>(false, kDepTileWarps);
   const size_t glb_smem = dep_smem_bytes<ORDER, R>(true, kGW);
   if (!attr_set) {
@@ -488,6 +726,7 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, Ctx& c
     cudaFuncSetAttribute(k_push_tile<R, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
     cudaFuncSetAttribute(kbox, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)box_smem);
     cudaFuncSetAttribute(kglb, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)glb_smem);
+    cudaFuncSetAttribute(kmma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mma_smem);
     attr_set = true;
   }
   {
@@ -496,7 +735,10 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, Ctx& c
   }
   {
     ScopedPhase ph(c, kPhaseDeposit);
-    if (variant == 1)
+    if (variant == 2)
+      kmma<<<n_tiles, kGW * 32, mma_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
+                                                     a.stray_count, a.deactivated);
+    else if (variant == 1)
       kglb<<<n_tiles, kGW * 32, glb_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
                                                      a.stray_count, a.deactivated);
     else
