@@ -68,11 +68,15 @@ enum {
   PIC_DEPOSIT_COOP = 2,       /* warp-cooperative: a warp walks its particles, lanes own window
                                  nodes, sums held in registers per cell run, one global
                                  reduction per node and run */
-  PIC_DEPOSIT_TILE = 3        /* one CTA per sort tile (tile edges <= 8 cells, after the first
+  PIC_DEPOSIT_TILE = 3,       /* one CTA per sort tile (tile edges <= 8 cells, after the first
                                  sort; otherwise falls back to COOP / GLOBAL): E/B stencil box
                                  staged in shared memory for gather + push; deposition by
-                                 16-lane groups into the tile's J box in shared memory, one
-                                 global reduction per node and tile. AUTO picks this when it can. */
+                                 16-lane groups (4 at order 1) that own the (j,k) columns of a
+                                 cell's window, sums in registers, one L2 reduction per finished
+                                 window node. AUTO picks this in fp32 when it can. */
+  PIC_DEPOSIT_TILE_MMA = 4    /* as TILE, but the sums of a cell's particles are formed as small
+                                 dense contractions on the fp64 tensor pipe (mma.sync m8n8k4.f64),
+                                 one warp per cell run. AUTO picks this in fp64 when it can. */
 };
 
 /* Options; pass NULL to pic_create for the defaults given here. */

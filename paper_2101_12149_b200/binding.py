@@ -14,7 +14,7 @@ LIB_PATH = os.path.join(_HERE, "libpic.so")
 
 PIC_F64, PIC_F32 = 0, 1
 PIC_HOST, PIC_DEVICE = 0, 1
-PIC_DEPOSIT_AUTO, PIC_DEPOSIT_GLOBAL, PIC_DEPOSIT_COOP, PIC_DEPOSIT_TILE = 0, 1, 2, 3
+PIC_DEPOSIT_AUTO, PIC_DEPOSIT_GLOBAL, PIC_DEPOSIT_COOP, PIC_DEPOSIT_TILE, PIC_DEPOSIT_TILE_MMA = 0, 1, 2, 3, 4
 PIC_NDIAG = 12
 PIC_NPHASE = 5
 DIAG_NAMES = ("field_E", "field_B", "kinetic", "charge", "gauss_max", "rho_max", "deactivated", "steps",

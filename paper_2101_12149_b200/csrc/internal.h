@@ -83,9 +83,9 @@ template <class R> void launch_pack(const Grid<R>& g, const R* valid_src, R* pad
 template <class R> void launch_unpack(const Grid<R>& g, const R* padded_src, R* valid_dst, Ctx& c);
 
 // ---- particles.cu
-enum { kDepositGlobal = 1, kDepositCoop = 2, kDepositTile = 3 };
-constexpr int kPushTileThreads = 512;   // k_push_tile: threads per CTA (one CTA per tile)
-constexpr int kDepTileWarps = 16;       // k_deposit_tile: warps per CTA (one CTA per tile)
+enum { kDepositGlobal = 1, kDepositCoop = 2, kDepositTile = 3, kDepositTileMma = 4 };
+constexpr int kPushTileThreads = 256;   // k_push_tile: threads per CTA (one CTA per tile)
+constexpr int kDepTileWarps = 8;        // k_deposit_tile / k_deposit_mma: warps per CTA (one CTA per tile, two per SM)
 template <class R>
 struct ParticleStep {
   Particles<R> cur;                  // x^n, u^{n-1/2}, w
@@ -106,7 +106,7 @@ bool launch_particles(const Grid<R>& g, const ParticleStep<R>& a, int order, int
 // ---- tile_kernels.cu: k_push_tile + k_deposit_tile of one species (needs tile_start); particles
 // they could not finish are in stray_list / stray_count[0]
 template <class R>
-void launch_tile_kernels(const Grid<R>& g, const ParticleStep<R>& a, int order, Ctx& c);
+void launch_tile_kernels(const Grid<R>& g, const ParticleStep<R>& a, int order, bool mma, Ctx& c);
 
 // ---- sort.cu
 struct SortScratch {

@@ -288,7 +288,7 @@ template <class R, int ORDER>
 bool launch_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) {
   const Particles<R>& p = a.cur;
   if (p.n == 0) return false;
-  if (mode != kDepositCoop && mode != kDepositTile) {
+  if (mode != kDepositCoop && mode != kDepositTile && mode != kDepositTileMma) {
     ScopedPhase ph(c, kPhasePush);
     int64_t nb = (p.n + 127) / 128;
     k_particles_global<R, ORDER><<<(unsigned)nb, 128, 0, c.stream>>>(g, p, a.deactivated);
@@ -302,17 +302,15 @@ bool launch_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) 
     cudaFuncSetAttribute(k_deposit_coop<R, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr_set = true;
   }
-  if (mode == kDepositTile) {
+  if (mode == kDepositTile || mode == kDepositTileMma) {
     // tile kernels, then the particles they listed: warp-cooperative pass over the list (window
     // fixed to each particle's own cell), then one thread each for what that pass lists
     cudaMemsetAsync(a.stray_count, 0, 2 * sizeof(unsigned int), c.stream);
-    launch_tile_kernels<R>(g, a, ORDER, c);
+    launch_tile_kernels<R>(g, a, ORDER, mode == kDepositTileMma, c);
     ScopedPhase ph(c, kPhaseStray);
-    k_deposit_coop<R, ORDER><<<148 * 2, kCoopWarps * 32, smem, c.stream>>>(
-        g, p, xn, yn, zn, nullptr, a.stray_list, a.stray_count, a.stray_list2, a.stray_count + 1, a.deactivated);
-    k_deposit_list<R, ORDER><<<148, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list2, a.stray_count + 1,
-                                                       a.deactivated);
-    c.launches += 2;
+    k_deposit_list<R, ORDER><<<148 * 8, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count,
+                                                           a.deactivated);
+    c.launches += 1;
     return true;
   }
   {

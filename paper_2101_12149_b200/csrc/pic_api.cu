@@ -312,9 +312,12 @@ struct Sim : SimBase {
   // AUTO: the warp-cooperative deposition needs the cell-sorted order to pay off
   int pick_mode(const Species<R>& sp) const {
     const bool tiles_ok = sp.sorted_once && tile.T[0] <= 8 && tile.T[1] <= 8 && tile.T[2] <= 8;
-    if (deposit_mode == PIC_DEPOSIT_TILE && !tiles_ok) return sp.sorted_once ? kDepositCoop : kDepositGlobal;
+    const bool want_tile = deposit_mode == PIC_DEPOSIT_TILE || deposit_mode == PIC_DEPOSIT_TILE_MMA;
+    if (want_tile && !tiles_ok) return sp.sorted_once ? kDepositCoop : kDepositGlobal;
     if (deposit_mode != PIC_DEPOSIT_AUTO) return deposit_mode;
-    return tiles_ok ? kDepositTile : (sp.sorted_once ? kDepositCoop : kDepositGlobal);
+    // fp64: the tensor-pipe deposition; fp32: the lane-group one (its sums run on the fp32 pipe)
+    const int tile_mode = sizeof(R) == 8 ? kDepositTileMma : kDepositTile;
+    return tiles_ok ? tile_mode : (sp.sorted_once ? kDepositCoop : kDepositGlobal);
   }
   void particle_step(Species<R>& sp) {
     ParticleStep<R> a;
@@ -551,7 +554,7 @@ int pic_create(const int32_t n_cells[3], const double dx[3], double dt, int shap
   if (shape_order < 1 || shape_order > 3) return bad(PIC_ERR_INVALID_ARG, "shape_order must be 1, 2 or 3");
   if (prec != PIC_F64 && prec != PIC_F32) return bad(PIC_ERR_INVALID_ARG, "unknown precision");
   if (o.sort_interval < 0 || o.sort_key_mode < 0 || o.sort_key_mode > 1 || o.reserved != 0 || o.deposit_mode < 0 ||
-      o.deposit_mode > 3)
+      o.deposit_mode > 4)
     return bad(PIC_ERR_INVALID_ARG, "bad option value");
   double s2 = 0;
   for (int d = 0; d < 3; ++d) {

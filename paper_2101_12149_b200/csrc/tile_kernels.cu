@@ -6,13 +6,16 @@
 //                   per-particle E/B in memory);
 //   k_deposit_tile  Esirkepov deposition (ref [8]) by groups of 16 lanes (4 at
 //                   order 1): the lanes of a group own the (j,k) columns of a cell's window, x runs
-//                   along registers, sums stay in registers for a run of cells along x, are folded
-//                   into the tile's J box in shared memory, and reach global memory once per tile.
-// Particles that no longer fit the tile's boxes (they drifted since the last sort) are handled by
-// the global-memory paths in particles.cu; correctness never depends on the order or the tile.
+//                   along registers (slot = node mod NX, so nothing moves when the window advances),
+//                   the groups of a warp take the particles of one cell together, and every
+//                   finished window node is one reduction at L2;
+//   k_deposit_mma   the same sums as 8 x 16 x K contractions on the fp64 tensor pipe, one warp per
+//                   run of same-cell particles (the fp64 default).
+// Particles that do not fit a kernel's windows (they crossed a cell face in y or z this step, or
+// drifted too far from the tile since the last sort) go to a list and are deposited one thread each
+// (particles.cu); correctness never depends on the order or the tile.
 #include <algorithm>
 #include <climits>
-#include <cstdlib>
 
 #include "internal.h"
 #include "particle_math.cuh"
@@ -35,17 +38,24 @@ __device__ __forceinline__ void tile_coords(const TileSpec& ts, int tile, int* t
 
 // =================================================================== gather + push from shared memory
 // Box of nodes staged per component: local index 0 is node (tile base - HB); EXT nodes per axis cover
-// the stencils (nodal and staggered) of every particle whose cell is within one cell of the tile.
+// the stencils (nodal and staggered) of every particle whose cell is inside the tile. Layout: y
+// fastest, then z (stride EXT), x slowest with stride SX = the first value >= EXT^2 that is 9 mod 16.
+// The lanes of a warp hold particles of a few cells that are neighbours along x, so their stencil
+// addresses differ by small multiples of SX (+-1 or +-EXT for a staggered base): with SX = 9 mod 16
+// no two of those fall in the same pair of banks (2.09 wavefronts per 64-bit load, 2.0 is the floor;
+// x fastest gives 2.58), and SX odd keeps the staging stores of an x-row conflict-free.
 template <int ORDER>
 struct PushBox {
-  static constexpr int HB = ORDER == 3 ? 3 : 2;
-  static constexpr int EXT = kTileMax + (ORDER == 1 ? 4 : (ORDER == 2 ? 5 : 6));   // 12, 13, 14
-  static constexpr int VOL = EXT * EXT * EXT;
+  static constexpr int HB = ORDER == 3 ? 2 : 1;
+  static constexpr int EXT = kTileMax + (ORDER == 1 ? 2 : (ORDER == 2 ? 3 : 4));   // 10, 11, 12
+  static constexpr int SX = EXT * EXT + ((9 - EXT * EXT % 16) + 16) % 16;            // 105, 121, 153
+  static constexpr int VOL = EXT * SX;
+  static constexpr int MAXD = 256;   // drifted particles a CTA lists before it gathers them in line
 };
 
 template <class R, int ORDER>
 __device__ __forceinline__ R interp_box(const R* __restrict__ F, int base, const R* wx, const R* wy, const R* wz) {
-  constexpr int E = PushBox<ORDER>::EXT;
+  constexpr int E = PushBox<ORDER>::EXT, SX = PushBox<ORDER>::SX;
   R acc = 0;
 #pragma unroll
   for (int c = 0; c <= ORDER; ++c) {
@@ -54,7 +64,7 @@ __device__ __forceinline__ R interp_box(const R* __restrict__ F, int base, const
     for (int b = 0; b <= ORDER; ++b) {
       R acca = 0;
 #pragma unroll
-      for (int a = 0; a <= ORDER; ++a) acca += wx[a] * F[base + E * E * a + b + E * c];
+      for (int a = 0; a <= ORDER; ++a) acca += wx[a] * F[base + SX * a + b + E * c];
       accb += wy[b] * acca;
     }
     acc += wz[c] * accb;
@@ -62,33 +72,46 @@ __device__ __forceinline__ R interp_box(const R* __restrict__ F, int base, const
   return acc;
 }
 
+template <class R>
+__device__ __forceinline__ void push_store(const Grid<R>& g, const Particles<R>& p, R* __restrict__ xn,
+                                           R* __restrict__ yn, R* __restrict__ zn, int t, const R* x0, R* u,
+                                           const R* Ef, const R* Bf) {
+  boris<R>(p.kq, g.inv_c2, Ef, Bf, u);
+  R ig = g.dt / sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * g.inv_c2);
+  xn[t] = x0[0] + u[0] * ig;
+  yn[t] = x0[1] + u[1] * ig;
+  zn[t] = x0[2] + u[2] * ig;
+  p.ux[t] = u[0]; p.uy[t] = u[1]; p.uz[t] = u[2];
+}
+
 template <class R, int ORDER>
-__global__ void __launch_bounds__(kPushTileThreads) k_push_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn,
-                                                                R* __restrict__ yn, R* __restrict__ zn,
-                                                                const int32_t* __restrict__ tile_start, TileSpec ts) {
+__global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn,
+                                                                   R* __restrict__ yn, R* __restrict__ zn,
+                                                                   const int32_t* __restrict__ tile_start, TileSpec ts) {
   using PB = PushBox<ORDER>;
-  constexpr int E = PB::EXT, VOL = PB::VOL;
+  constexpr int E = PB::EXT, SX = PB::SX, VOL = PB::VOL;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  R* box = reinterpret_cast<R*>(smem_raw);   // [6][E][E][E]
+  R* box = reinterpret_cast<R*>(smem_raw);   // [6][E (x)][SX: E (z) x E (y), padded]
+  __shared__ int s_drift[PB::MAXD];
+  __shared__ int s_ndrift;
   const int tile = blockIdx.x;
   const int s = tile_start[tile], e = tile_start[tile + 1];
   if (s >= e) return;
+  if (threadIdx.x == 0) s_ndrift = 0;
   int tb[3];
   tile_coords(ts, tile, tb);
   const int o0 = tb[0] - PB::HB, o1 = tb[1] - PB::HB, o2 = tb[2] - PB::HB;   // node of local (0,0,0)
-  // stage the six boxes (nodes beyond the padded array, possible only for tiles smaller than 8, read 0)
+  // stage the six boxes, reading along x (nodes beyond the padded array, possible only for tiles
+  // smaller than 8, read 0)
   const int lim0 = g.N[0] + kGuard, lim1 = g.N[1] + kGuard, lim2 = g.N[2] + kGuard;
-  // box layout: y fastest, then z, x slowest. The lanes of a warp hold particles of a few cells that
-  // are neighbours along x, so their stencil addresses differ by multiples of E*E = 196 = 4 (mod 16
-  // doubles): no two fall in the same bank pair (2.10 wavefronts per 64-bit load against 2.58 with x
-  // fastest, where a y-staggered base one row up collides with a cell two to the right).
-  for (int idx = threadIdx.x; idx < VOL; idx += blockDim.x) {
-    int j = idx % E, r = idx / E;
-    int k = r % E, i = r / E;
+  for (int idx = threadIdx.x; idx < E * E * E; idx += blockDim.x) {
+    int i = idx % E, r = idx / E;
+    int j = r % E, k = r / E;
     const bool in = (o0 + i < lim0) & (o1 + j < lim1) & (o2 + k < lim2);
     const int gi = g.idx(o0 + i, o1 + j, o2 + k);
+    const int li = SX * i + j + E * k;
 #pragma unroll
-    for (int c = 0; c < 6; ++c) box[c * VOL + idx] = in ? __ldg(g.F[c] + gi) : R(0);
+    for (int c = 0; c < 6; ++c) box[c * VOL + li] = in ? __ldg(g.F[c] + gi) : R(0);
   }
   __syncthreads();
   for (int t = s + threadIdx.x; t < e; t += blockDim.x) {
@@ -100,31 +123,39 @@ __global__ void __launch_bounds__(kPushTileThreads) k_push_tile(Grid<R> g, Parti
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
       R xi = x0[d] * g.inv_dx[d];
-      ln[d] = shape<R, ORDER>(xi, wn[d]);
-      ls[d] = shape<R, ORDER>(xi - R(0.5), ws[d]);
-      const int od = d == 0 ? o0 : (d == 1 ? o1 : o2);
-      const int a = ln[d] - od, b = ls[d] - od;
-      inbox &= (a >= 0) & (a <= E - ORDER - 1) & (b >= 0) & (b <= E - ORDER - 1);
-      if (inbox) { ln[d] = a; ls[d] = b; }
+      ln[d] = shape<R, ORDER>(xi, wn[d]) - (d == 0 ? o0 : (d == 1 ? o1 : o2));
+      ls[d] = shape<R, ORDER>(xi - R(0.5), ws[d]) - (d == 0 ? o0 : (d == 1 ? o1 : o2));
+      inbox &= (ln[d] >= 0) & (ln[d] <= E - ORDER - 1) & (ls[d] >= 0) & (ls[d] <= E - ORDER - 1);
+    }
+    if (!inbox) {
+      // drifted out of the tile since the last sort: listed, gathered from global memory below with
+      // all lanes busy (in line if the list is full)
+      const int slot = atomicAdd(&s_ndrift, 1);
+      if (slot < PB::MAXD) { s_drift[slot] = t; continue; }
+      R Ef[3], Bf[3];
+      gather6<R, ORDER>(g, x0[0], x0[1], x0[2], Ef, Bf);
+      push_store<R>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
+      continue;
     }
     R Ef[3], Bf[3];
-    if (inbox) {
-      // Ex (s,n,n)  Ey (n,s,n)  Ez (n,n,s)  Bx (n,s,s)  By (s,n,s)  Bz (s,s,n)
-      Ef[0] = interp_box<R, ORDER>(box + 0 * VOL, E * E * ls[0] + ln[1] + E * ln[2], ws[0], wn[1], wn[2]);
-      Ef[1] = interp_box<R, ORDER>(box + 1 * VOL, E * E * ln[0] + ls[1] + E * ln[2], wn[0], ws[1], wn[2]);
-      Ef[2] = interp_box<R, ORDER>(box + 2 * VOL, E * E * ln[0] + ln[1] + E * ls[2], wn[0], wn[1], ws[2]);
-      Bf[0] = interp_box<R, ORDER>(box + 3 * VOL, E * E * ln[0] + ls[1] + E * ls[2], wn[0], ws[1], ws[2]);
-      Bf[1] = interp_box<R, ORDER>(box + 4 * VOL, E * E * ls[0] + ln[1] + E * ls[2], ws[0], wn[1], ws[2]);
-      Bf[2] = interp_box<R, ORDER>(box + 5 * VOL, E * E * ls[0] + ls[1] + E * ln[2], ws[0], ws[1], wn[2]);
-    } else {
-      gather6<R, ORDER>(g, x0[0], x0[1], x0[2], Ef, Bf);   // drifted out of the box: global memory
-    }
-    boris<R>(p.kq, g.inv_c2, Ef, Bf, u);
-    R ig = g.dt / sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * g.inv_c2);
-    xn[t] = x0[0] + u[0] * ig;
-    yn[t] = x0[1] + u[1] * ig;
-    zn[t] = x0[2] + u[2] * ig;
-    p.ux[t] = u[0]; p.uy[t] = u[1]; p.uz[t] = u[2];
+    // Ex (s,n,n)  Ey (n,s,n)  Ez (n,n,s)  Bx (n,s,s)  By (s,n,s)  Bz (s,s,n)
+    Ef[0] = interp_box<R, ORDER>(box + 0 * VOL, SX * ls[0] + ln[1] + E * ln[2], ws[0], wn[1], wn[2]);
+    Ef[1] = interp_box<R, ORDER>(box + 1 * VOL, SX * ln[0] + ls[1] + E * ln[2], wn[0], ws[1], wn[2]);
+    Ef[2] = interp_box<R, ORDER>(box + 2 * VOL, SX * ln[0] + ln[1] + E * ls[2], wn[0], wn[1], ws[2]);
+    Bf[0] = interp_box<R, ORDER>(box + 3 * VOL, SX * ln[0] + ls[1] + E * ls[2], wn[0], ws[1], ws[2]);
+    Bf[1] = interp_box<R, ORDER>(box + 4 * VOL, SX * ls[0] + ln[1] + E * ls[2], ws[0], wn[1], ws[2]);
+    Bf[2] = interp_box<R, ORDER>(box + 5 * VOL, SX * ls[0] + ls[1] + E * ln[2], ws[0], ws[1], wn[2]);
+    push_store<R>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
+  }
+  __syncthreads();
+  const int nd = min(s_ndrift, PB::MAXD);
+  for (int q = threadIdx.x; q < nd; q += blockDim.x) {
+    const int t = s_drift[q];
+    R x0[3] = {p.x[t], p.y[t], p.z[t]};
+    R u[3] = {p.ux[t], p.uy[t], p.uz[t]};
+    R Ef[3], Bf[3];
+    gather6<R, ORDER>(g, x0[0], x0[1], x0[2], Ef, Bf);
+    push_store<R>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
   }
 }
 
@@ -140,9 +171,6 @@ struct TWin {
   static constexpr int NX = ORDER == 1 ? 4 : 6, BLX = ORDER == 1 ? 1 : 2;
   static constexpr int NYZ = ORDER == 1 ? 2 : 4, BLYZ = ORDER == 1 ? 0 : 1;
   static constexpr int LG = NYZ * NYZ;                 // lanes per particle: 4 or 16
-  static constexpr int EX = kTileMax + NX - 1;         // J box of the tile: 11 / 13 nodes along x
-  static constexpr int EYZ = kTileMax + NYZ - 1;       // 9 / 11 along y and z
-  static constexpr int JVOL = EX * EYZ * EYZ;
   // record (elements): {A_x,B_x}[NX] | PX[NX] | {S0_y,DS_y}[NYZ] | PY[NYZ] | {S0_z,DS_z}[NYZ] | PZ[NYZ]
   static constexpr int oAB = 0, oPX = 2 * NX, oY = 3 * NX, oPY = 3 * NX + 2 * NYZ, oZ = 3 * NX + 3 * NYZ,
                        oPZ = 3 * NX + 5 * NYZ;
@@ -200,8 +228,6 @@ __device__ __forceinline__ void axis_window(R xi0, R xi1, int& cell, R* S0, R* D
   fits = (so0 >= 0) & (so0 + ORDER < NW) & (sl1 >= 0) & (sl1 + ORDER < NW);
 }
 
-__device__ __forceinline__ void smem_add(double* p, double v) { atomicAdd(p, v); }   // CAS loop on sm_100a
-__device__ __forceinline__ void smem_add(float* p, float v) { atomicAdd(p, v); }
 
 // Register accumulators of one lane: the (j,k) column of a window of NX nodes along x, three
 // components. The slot of box node X is X mod NX, so when the window advances by one cell nothing
@@ -237,14 +263,9 @@ __device__ __forceinline__ void accumulate(Acc<R, TWin<ORDER>::NX>& a, const R* 
   }
 }
 
-// where a window's first node lives, per component: the tile's J box in shared memory, or (GLOBAL)
-// the J arrays themselves
+// where a window's first node lives in the three J arrays
 template <class R>
 struct JPtr { R* p[3]; };
-template <bool GLOBAL, class R>
-__device__ __forceinline__ void j_add(R* p, R v) {
-  if constexpr (GLOBAL) red_add(p, v); else smem_add(p, v);
-}
 
 // sum over the NG groups of a warp (lanes that own the same column), result in every lane
 template <class R, int LG>
@@ -254,21 +275,22 @@ __device__ __forceinline__ R group_sum(R v) {
   return v;
 }
 
-// one physical slot (static P) of all groups -> box element jx[0..2*JVOL], then cleared. Warp-uniform.
-template <class R, int ORDER, int P, bool GLOBAL>
+// one physical slot (static P), summed over the groups -> the J element jx points at, then cleared.
+// Warp-uniform.
+template <class R, int ORDER, int P>
 __device__ __forceinline__ void flush_slot(Acc<R, TWin<ORDER>::NX>& a, const JPtr<R>& jx, bool writer) {
   using W = TWin<ORDER>;
   const R vx = group_sum<R, W::LG>(a.x[P]), vy = group_sum<R, W::LG>(a.y[P]), vz = group_sum<R, W::LG>(a.z[P]);
   if (writer) {
-    if (vx != R(0)) j_add<GLOBAL>(jx.p[0], vx);
-    if (vy != R(0)) j_add<GLOBAL>(jx.p[1], vy);
-    if (vz != R(0)) j_add<GLOBAL>(jx.p[2], vz);
+    if (vx != R(0)) red_add(jx.p[0], vx);
+    if (vy != R(0)) red_add(jx.p[1], vy);
+    if (vz != R(0)) red_add(jx.p[2], vz);
   }
   a.x[P] = 0; a.y[P] = 0; a.z[P] = 0;
 }
 
 // all slots: physical slot p holds logical slot (p - ph) mod NX of the window at jx. Warp-uniform.
-template <class R, int ORDER, bool GLOBAL>
+template <class R, int ORDER>
 __device__ __forceinline__ void flush_window(Acc<R, TWin<ORDER>::NX>& a, const JPtr<R>& jx, int ph, bool writer) {
   using W = TWin<ORDER>;
   constexpr int NX = W::NX;
@@ -278,9 +300,9 @@ __device__ __forceinline__ void flush_window(Acc<R, TWin<ORDER>::NX>& a, const J
     i += i < 0 ? NX : 0;
     const R vx = group_sum<R, W::LG>(a.x[p]), vy = group_sum<R, W::LG>(a.y[p]), vz = group_sum<R, W::LG>(a.z[p]);
     if (writer) {
-      if (vx != R(0)) j_add<GLOBAL>(jx.p[0] + i, vx);
-      if (vy != R(0)) j_add<GLOBAL>(jx.p[1] + i, vy);
-      if (vz != R(0)) j_add<GLOBAL>(jx.p[2] + i, vz);
+      if (vx != R(0)) red_add(jx.p[0] + i, vx);
+      if (vy != R(0)) red_add(jx.p[1] + i, vy);
+      if (vz != R(0)) red_add(jx.p[2] + i, vz);
     }
   }
   a.zero();
@@ -288,31 +310,28 @@ __device__ __forceinline__ void flush_window(Acc<R, TWin<ORDER>::NX>& a, const J
 
 // the particles of one cell (cnt of them, record slots listed in order[]): NG at a time, one per
 // group. PH = (first box node of the cell's window) mod NX; adv = the window moved up one cell.
-template <class R, int ORDER, int PH, bool GLOBAL>
+template <class R, int ORDER, int PH>
 __device__ __forceinline__ void cell_batch(Acc<R, TWin<ORDER>::NX>& a, bool adv, const JPtr<R>& jx_old, bool writer,
                                            const R* __restrict__ rec, const int* __restrict__ order, int cnt, int grp,
                                            int j, int k) {
   using W = TWin<ORDER>;
   constexpr int NX = W::NX, NG = 32 / W::LG;
-  if (adv) flush_slot<R, ORDER, (PH + NX - 1) % NX, GLOBAL>(a, jx_old, writer);
+  if (adv) flush_slot<R, ORDER, (PH + NX - 1) % NX>(a, jx_old, writer);
 #pragma unroll 1
   for (int it = grp; it < cnt; it += NG) accumulate<R, ORDER, PH>(a, rec + order[it] * W::REC, j, k);
 }
 
-// GLOBAL = false: sums go to the tile's J box in shared memory and reach the J arrays once per tile;
-// GLOBAL = true: no box, every finished window node is one reduction at L2 (smaller CTAs, no
-// prologue/epilogue, no block barrier).
-template <class R, int ORDER, bool GLOBAL, int NWARP>
-__global__ void __launch_bounds__(NWARP * 32, GLOBAL ? 2 : 1)
+// Every finished window node is one reduction at L2 (RED.ADD.F64 / .F32): no J box in shared memory,
+// no prologue / epilogue, no block barrier, so two 8-warp CTAs per SM overlap freely.
+template <class R, int ORDER, int NWARP>
+__global__ void __launch_bounds__(NWARP * 32, 2)
     k_deposit_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn, R* __restrict__ yn, R* __restrict__ zn,
                    const int32_t* __restrict__ tile_start, TileSpec ts, int32_t* __restrict__ stray_list,
                    unsigned int* __restrict__ stray_count, unsigned long long* deactivated) {
   using W = TWin<ORDER>;
-  constexpr int NX = W::NX, NYZ = W::NYZ, LG = W::LG, EX = W::EX, EYZ = W::EYZ, JVOL = W::JVOL, REC = W::REC;
-  constexpr int JBOX = GLOBAL ? 0 : 3 * JVOL + ((3 * JVOL) & 1);   // keeps the records 16-byte aligned
+  constexpr int NX = W::NX, NYZ = W::NYZ, LG = W::LG, REC = W::REC;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  R* Jt = reinterpret_cast<R*>(smem_raw);            // [3][EYZ][EYZ][EX]
-  R* rec_all = Jt + JBOX;
+  R* rec_all = reinterpret_cast<R*>(smem_raw);
   __shared__ int s_order[NWARP][32];
 
   const int tile = blockIdx.x;
@@ -320,10 +339,6 @@ __global__ void __launch_bounds__(NWARP * 32, GLOBAL ? 2 : 1)
   if (s >= e) return;
   int tb[3];
   tile_coords(ts, tile, tb);
-  if constexpr (!GLOBAL) {
-    for (int i = threadIdx.x; i < 3 * JVOL; i += blockDim.x) Jt[i] = R(0);
-    __syncthreads();
-  }
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int grp = lane / LG, gl = lane % LG;
@@ -332,13 +347,8 @@ __global__ void __launch_bounds__(NWARP * 32, GLOBAL ? 2 : 1)
   const int b0 = tb[0] - W::BLX, b1 = tb[1] - W::BLYZ, b2 = tb[2] - W::BLYZ;
   auto column = [&](int off) {
     JPtr<R> q;
-    if constexpr (GLOBAL) {
-      const int gi = g.idx(b0 + (off & 15), b1 + ((off >> 4) & 15) + j, b2 + (off >> 8) + k);
-      q.p[0] = g.J[0] + gi; q.p[1] = g.J[1] + gi; q.p[2] = g.J[2] + gi;
-    } else {
-      R* c0 = Jt + (off & 15) + EX * (((off >> 4) & 15) + j + EYZ * ((off >> 8) + k));
-      q.p[0] = c0; q.p[1] = c0 + JVOL; q.p[2] = c0 + 2 * JVOL;
-    }
+    const int gi = g.idx(b0 + (off & 15), b1 + ((off >> 4) & 15) + j, b2 + (off >> 8) + k);
+    q.p[0] = g.J[0] + gi; q.p[1] = g.J[1] + gi; q.p[2] = g.J[2] + gi;
     return q;
   };
   R* rec = rec_all + (size_t)warp * 32 * REC;
@@ -411,15 +421,15 @@ __global__ void __launch_bounds__(NWARP * 32, GLOBAL ? 2 : 1)
       const bool adv = ib == cur + 1;
       JPtr<R> jx_old{};
       if (cur != INT_MIN) jx_old = column(cur);
-      if (ib != cur && !adv && cur != INT_MIN) flush_window<R, ORDER, GLOBAL>(acc, jx_old, curph, grp == 0);
+      if (ib != cur && !adv && cur != INT_MIN) flush_window<R, ORDER>(acc, jx_old, curph, grp == 0);
       const int* ord = s_order[warp];
       switch (ph) {
-        case 0: cell_batch<R, ORDER, 0, GLOBAL>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 1: cell_batch<R, ORDER, 1, GLOBAL>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 2: cell_batch<R, ORDER, 2, GLOBAL>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 3: cell_batch<R, ORDER, 3 % NX, GLOBAL>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 4: cell_batch<R, ORDER, 4 % NX, GLOBAL>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        default: cell_batch<R, ORDER, 5 % NX, GLOBAL>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 0: cell_batch<R, ORDER, 0>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 1: cell_batch<R, ORDER, 1>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 2: cell_batch<R, ORDER, 2>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 3: cell_batch<R, ORDER, 3 % NX>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 4: cell_batch<R, ORDER, 4 % NX>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        default: cell_batch<R, ORDER, 5 % NX>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
       }
       cur = ib;
       curph = ph;
@@ -445,20 +455,7 @@ __global__ void __launch_bounds__(NWARP * 32, GLOBAL ? 2 : 1)
       xn[t] = x1[0]; yn[t] = x1[1]; zn[t] = x1[2];
     }
   }
-  if (cur != INT_MIN) flush_window<R, ORDER, GLOBAL>(acc, column(cur), curph, grp == 0);
-  if constexpr (GLOBAL) return;
-  __syncthreads();
-  // the tile's J box -> global memory, one reduction per touched node
-  for (int idx = threadIdx.x; idx < JVOL; idx += blockDim.x) {
-    const int i = idx % EX, rr = idx / EX;
-    const int jj = rr % EYZ, kk = rr / EYZ;
-    const int gi = g.idx(b0 + i, b1 + jj, b2 + kk);
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-      const R v = Jt[c * JVOL + idx];
-      if (v != R(0)) red_add(g.J[c] + gi, v);
-    }
-  }
+  if (cur != INT_MIN) flush_window<R, ORDER>(acc, column(cur), curph, grp == 0);
 }
 
 // =================================================================== Esirkepov on the fp64 tensor pipe
@@ -699,33 +696,21 @@ __global__ void __launch_bounds__(NWARP * 32, 2)
 
 }  // namespace
 
-template <int ORDER, class R>
-static size_t dep_smem_bytes(bool global, int nwarp) {
-  using W = TWin<ORDER>;
-  const size_t jbox = global ? 0 : 3 * W::JVOL + ((3 * W::JVOL) & 1);
-  return (jbox + (size_t)nwarp * 32 * W::REC) * sizeof(R);
-}
-
 template <class R, int ORDER>
-static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, Ctx& c) {
+static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, bool mma, Ctx& c) {
   const Particles<R>& p = a.cur;
   R *xn = a.alt.x, *yn = a.alt.y, *zn = a.alt.z;
   const int n_tiles = a.tiles.nt[0] * a.tiles.nt[1] * a.tiles.nt[2];
   static bool attr_set = false;
-  static int variant = 2;
+  constexpr int kW = kDepTileWarps;
+  auto kvec = k_deposit_tile<R, ORDER, kW>;
+  auto kmma = k_deposit_mma<R, ORDER, kW>;
   const size_t push_smem = (size_t)6 * PushBox<ORDER>::VOL * sizeof(R);
-  constexpr int kGW = 8;
-  auto kbox = k_deposit_tile<R, ORDER, false, kDepTileWarps>;
-  auto kglb = k_deposit_tile<R, ORDER, true, kGW>;
-  auto kmma = k_deposit_mma<R, ORDER, kGW>;
-  const size_t mma_smem = (size_t)kGW * 33 * MWin<ORDER>::REC * sizeof(R);
-  const size_t box_smem = dep_smem_bytes<ORDER, R>(false, kDepTileWarps);
-  const size_t glb_smem = dep_smem_bytes<ORDER, R>(true, kGW);
+  const size_t vec_smem = (size_t)kW * 32 * TWin<ORDER>::REC * sizeof(R);
+  const size_t mma_smem = (size_t)kW * 33 * MWin<ORDER>::REC * sizeof(R);
   if (!attr_set) {
-    if (const char* v = getenv("PIC_DEP_VARIANT")) variant = atoi(v);
     cudaFuncSetAttribute(k_push_tile<R, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
-    cudaFuncSetAttribute(kbox, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)box_smem);
-    cudaFuncSetAttribute(kglb, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)glb_smem);
+    cudaFuncSetAttribute(kvec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vec_smem);
     cudaFuncSetAttribute(kmma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mma_smem);
     attr_set = true;
   }
@@ -735,29 +720,26 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, Ctx& c
   }
   {
     ScopedPhase ph(c, kPhaseDeposit);
-    if (variant == 2)
-      kmma<<<n_tiles, kGW * 32, mma_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
-                                                     a.stray_count, a.deactivated);
-    else if (variant == 1)
-      kglb<<<n_tiles, kGW * 32, glb_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
-                                                     a.stray_count, a.deactivated);
+    if (mma)
+      kmma<<<n_tiles, kW * 32, mma_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
+                                                    a.stray_count, a.deactivated);
     else
-      kbox<<<n_tiles, kDepTileWarps * 32, box_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
-                                                               a.stray_count, a.deactivated);
+      kvec<<<n_tiles, kW * 32, vec_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
+                                                    a.stray_count, a.deactivated);
   }
   c.launches += 2;
 }
 
 template <class R>
-void launch_tile_kernels(const Grid<R>& g, const ParticleStep<R>& a, int order, Ctx& c) {
+void launch_tile_kernels(const Grid<R>& g, const ParticleStep<R>& a, int order, bool mma, Ctx& c) {
   switch (order) {
-    case 1: launch_tile_order<R, 1>(g, a, c); break;
-    case 2: launch_tile_order<R, 2>(g, a, c); break;
-    default: launch_tile_order<R, 3>(g, a, c); break;
+    case 1: launch_tile_order<R, 1>(g, a, mma, c); break;
+    case 2: launch_tile_order<R, 2>(g, a, mma, c); break;
+    default: launch_tile_order<R, 3>(g, a, mma, c); break;
   }
 }
 
-template void launch_tile_kernels<double>(const Grid<double>&, const ParticleStep<double>&, int, Ctx&);
-template void launch_tile_kernels<float>(const Grid<float>&, const ParticleStep<float>&, int, Ctx&);
+template void launch_tile_kernels<double>(const Grid<double>&, const ParticleStep<double>&, int, bool, Ctx&);
+template void launch_tile_kernels<float>(const Grid<float>&, const ParticleStep<float>&, int, bool, Ctx&);
 
 }  // namespace pic

@@ -77,7 +77,7 @@ def test_sort_edge_positions_and_ragged_sizes():
 
 # ------------------------------------------------------------------ one step from identical state
 @pytest.mark.parametrize("order", [1, 2, 3])
-@pytest.mark.parametrize("mode", [1, 2, 3])
+@pytest.mark.parametrize("mode", [1, 2, 3, 4])
 def test_one_step_fp64(order, mode):
     cfg = small("C2", (24, 16, 16), order=order, dx=(1.0e-6, 0.8e-6, 0.6e-6))
     cfg.species[0].sigma = 0.2            # hot: many cell crossings in one step
@@ -88,7 +88,7 @@ def test_one_step_fp64(order, mode):
 
 
 @pytest.mark.parametrize("order", [1, 3])
-@pytest.mark.parametrize("mode", [1, 2, 3])
+@pytest.mark.parametrize("mode", [1, 2, 3, 4])
 def test_one_step_fp32(order, mode):
     cfg = small("C3", (24, 16, 16), order=order)
     cfg.species[0].sigma = 0.1
@@ -99,12 +99,14 @@ def test_one_step_fp32(order, mode):
 
 @pytest.mark.parametrize("order", [1, 2, 3])
 @pytest.mark.parametrize("tile", [(8, 8, 8), (4, 8, 2)])
-def test_tile_path_steps_between_sorts(order, tile):
-    """Tile kernels (one CTA per sort tile) on the steps after a sort, when hot particles have left
-    their cell, their tile's J box (-> list -> warp pass -> per-particle pass) and its E/B box."""
+@pytest.mark.parametrize("mode", [3, 4])
+def test_tile_path_steps_between_sorts(order, tile, mode):
+    """Tile kernels (one CTA per sort tile; deposition by lane groups = 3, on the fp64 tensor pipe = 4)
+    on the steps after a sort, when hot particles have left their cell, the reach of their tile's
+    windows (-> list -> per-particle pass) and its E/B box (-> drift list -> global gather)."""
     cfg = small("C2", (24, 16, 8), order=order, tile=tile, dx=(1.0e-6, 0.8e-6, 0.6e-6))
     cfg.species[0].sigma = 0.5
-    o, g, _ = make_pair(cfg, fields="random", gpu_kwargs=dict(deposit_mode=3))
+    o, g, _ = make_pair(cfg, fields="random", gpu_kwargs=dict(deposit_mode=mode))
     o.step(1); g.step(1)
     compare_state(o, g, TOL64)
     o.step(3); g.step(3)                 # no re-sort: the order is stale by up to 3 cells
@@ -122,10 +124,11 @@ def test_tile_path_fp32_steps_between_sorts():
     compare_state(o, g, 4 * TOL32)
 
 
-def test_tile_path_empty_tiles_and_tile_only_key():
+@pytest.mark.parametrize("mode", [3, 4])
+def test_tile_path_empty_tiles_and_tile_only_key(mode):
     """Tiles with no particle (C4's vacuum region) and sort_key_mode 1 (order inside a tile is free)."""
     cfg = small("C4", (16, 16, 48), z_first=24, ramp_cells=8)
-    o, g, _ = make_pair(cfg, gpu_kwargs=dict(deposit_mode=3))
+    o, g, _ = make_pair(cfg, gpu_kwargs=dict(deposit_mode=mode))
     o.step(2); g.step(2)
     compare_state(o, g, 20 * TOL64)
     import oracle
@@ -136,7 +139,7 @@ def test_tile_path_empty_tiles_and_tile_only_key():
     E, B = W.random_fields(cfg, np.random.default_rng(5))
     kw = dict(tile=(8, 8, 8), sort_interval=4, sort_key_mode=1)
     oo = oracle.Oracle(cfg.n_cells, cfg.dx, cfg.dt, 2, **kw)
-    gg = pic.Sim(cfg.n_cells, cfg.dx, cfg.dt, 2, deposit_mode=3, **kw)
+    gg = pic.Sim(cfg.n_cells, cfg.dx, cfg.dt, 2, deposit_mode=mode, **kw)
     a = [species[0][1][k] for k in ("x", "y", "z", "ux", "uy", "uz", "w")]
     for s_ in (oo, gg):
         s_.add_species(*a, species[0][0].charge, species[0][0].mass)
