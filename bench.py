@@ -385,8 +385,10 @@ def run_ours(args):
     alu_peak = N_SM * per_clk * 2 * sm_max * 1e6 / 1e12          # TFLOP/s at the maximum SM clock
     per_launch = {k: (v[0] / v[1] if v[1] else 0.0) for k, v in phases.items()}
     n_species = len(cfg.species)
-    kern = {"push": ("k_push (gather + Boris push)", m["push_bytes"], m["push_flops"]),
-            "deposit": ("k_deposit_coop (Esirkepov)", m["deposit_bytes"], m["deposit_flops"])}
+    dep_name = ("k_deposit_mma (Esirkepov, fp64 tensor pipe)" if cfg.dtype == "f64" and args.deposit_mode in (0, 4)
+                else "k_deposit_tile / k_deposit_coop (Esirkepov, lane groups)")
+    kern = {"push": ("k_push_tile (gather + Boris push)", m["push_bytes"], m["push_flops"]),
+            "deposit": (dep_name, m["deposit_bytes"], m["deposit_flops"])}
     fused = phases["deposit"][1] == 0
     if fused:
         kern = {"push": ("k_particles_global (gather + push + deposit)", m["fused_bytes"],
@@ -436,7 +438,7 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=8)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C2", choices=sorted(W.CONFIGS))
-    ap.add_argument("--deposit-mode", type=int, default=0, help="PIC_DEPOSIT_* (0 auto, 1 global, 2 cooperative)")
+    ap.add_argument("--deposit-mode", type=int, default=0, help="PIC_DEPOSIT_* (0 auto, 1 global, 2 cooperative, 3 tile, 4 tile + fp64 tensor pipe)")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs: device-resident leg only")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs: do not time the oracle")
     ap.add_argument("--traffic", type=float, default=None,

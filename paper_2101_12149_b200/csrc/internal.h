@@ -85,6 +85,8 @@ template <class R> void launch_unpack(const Grid<R>& g, const R* padded_src, R* 
 // ---- particles.cu
 enum { kDepositGlobal = 1, kDepositCoop = 2, kDepositTile = 3, kDepositTileMma = 4 };
 constexpr int kPushTileThreads = 256;   // k_push_tile: threads per CTA (one CTA per tile)
+constexpr int kDepMmaWarps = 4;         // k_deposit_mma: warps per CTA (one CTA per tile) ...
+constexpr int kDepMmaCtas = 5;          // ... and CTAs per SM the register budget is set for (20 warps per SM)
 constexpr int kDepTileWarps = 8;        // k_deposit_tile / k_deposit_mma: warps per CTA (one CTA per tile, two per SM)
 template <class R>
 struct ParticleStep {

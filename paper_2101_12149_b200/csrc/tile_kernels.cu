@@ -479,11 +479,9 @@ struct MWin {
   static constexpr int NCOL = NYZ * NYZ;              // 16 (orders 2, 3) or 4 (order 1)
   static constexpr int NB = NCOL > 8 ? NCOL / 8 : 1;  // 8-column blocks of C
   static constexpr int KSTEP = NYZ == 4 ? 2 : 0;      // k advances by this from one column block to the next
-  // record (elements): {A_x,B_x}[NX] | PX[NX] | {al_y,be_y}[NYZ] | {S0_y,DS_y}[NYZ] | PY[NYZ] |
-  //                    {S0_z,DS_z}[NYZ] | PZ[NYZ]
-  static constexpr int oAB = 0, oPX = 2 * NX, oYab = 3 * NX, oY = oYab + 2 * NYZ, oPY = oY + 2 * NYZ,
-                       oZ = oPY + NYZ, oPZ = oZ + 2 * NYZ;
-  static constexpr int RAW = oPZ + NYZ;                            // 50 / 28
+  // record (elements): {A_x,B_x}[NX] | PX[NX] | {S0_y,DS_y}[NYZ] | PY[NYZ] | {S0_z,DS_z}[NYZ] | PZ[NYZ]
+  static constexpr int oAB = 0, oPX = 2 * NX, oY = 3 * NX, oPY = oY + 2 * NYZ, oZ = oPY + NYZ, oPZ = oZ + 2 * NYZ;
+  static constexpr int RAW = oPZ + NYZ;                            // 42 / 24
   static constexpr int REC = (RAW / 2) % 2 == 1 ? RAW : RAW + 2;   // REC/2 odd: conflict-free pair stores
 };
 
@@ -499,8 +497,8 @@ struct CFrag {
   }
 };
 
-template <class R, int ORDER, int NWARP>
-__global__ void __launch_bounds__(NWARP * 32, 2)
+template <class R, int ORDER, int NWARP, int MINB>
+__global__ void __launch_bounds__(NWARP * 32, MINB)
     k_deposit_mma(Grid<R> g, Particles<R> p, R* __restrict__ xn, R* __restrict__ yn, R* __restrict__ zn,
                   const int32_t* __restrict__ tile_start, TileSpec ts, int32_t* __restrict__ stray_list,
                   unsigned int* __restrict__ stray_count, unsigned long long* deactivated) {
@@ -526,7 +524,7 @@ __global__ void __launch_bounds__(NWARP * 32, 2)
   // B operands: this lane supplies column gq (+ 8 per block) = (jB, kB + KSTEP * block)
   const bool colok = gq < W::NCOL;
   const int jB = colok ? gq % NYZ : 0, kB = colok ? gq / NYZ : 0;
-  const int offYab = W::oYab + 2 * jB, offY = W::oY + 2 * jB, offPY = W::oPY + jB, offZ = W::oZ + 2 * kB,
+  const int offY = W::oY + 2 * jB, offPY = W::oPY + jB, offZ = W::oZ + 2 * kB,
             offPZ = W::oPZ + kB;
   // C fragments: this lane holds columns 2t + {0,1} (+ 8 per block) of row gq
   int coff[NB][2];
@@ -610,8 +608,6 @@ __global__ void __launch_bounds__(NWARP * 32, 2)
         }
 #pragma unroll
         for (int i = 0; i < NYZ; ++i) {
-          *reinterpret_cast<Pair2<R>*>(rr + W::oYab + 2 * i) =
-              Pair2<R>{S0y[i] + half * DSy[i], half * S0y[i] + third * DSy[i]};
           *reinterpret_cast<Pair2<R>*>(rr + W::oY + 2 * i) = Pair2<R>{S0y[i], DSy[i]};
           *reinterpret_cast<Pair2<R>*>(rr + W::oZ + 2 * i) = Pair2<R>{S0z[i], DSz[i]};
           py += DSy[i]; pz += DSz[i];
@@ -645,11 +641,12 @@ __global__ void __launch_bounds__(NWARP * 32, 2)
           const R* rr = rec + (b + t < s1 ? b + t : 32) * REC;      // slot 32: the all-zero record
           const R* ra = rowok ? rr : zrec;
           const double a = ra[offPX];
-          const Pair2<R> ab = *reinterpret_cast<const Pair2<R>*>(rr + offYab);
+          const Pair2<R> yv = *reinterpret_cast<const Pair2<R>*>(rr + offY);
+          const double al = fma(0.5, (double)yv.b, (double)yv.a), be = fma(0.5, (double)yv.a, (double)yv.b * (1.0 / 3.0));
 #pragma unroll
           for (int nb = 0; nb < NB; ++nb) {
             const Pair2<R> zv = *reinterpret_cast<const Pair2<R>*>(rr + offZ + 2 * W::KSTEP * nb);
-            const double cx = fma((double)zv.a, (double)ab.a, (double)zv.b * (double)ab.b);
+            const double cx = fma((double)zv.a, al, (double)zv.b * be);
             dmma_884(C.x[nb][0], C.x[nb][1], a, colok ? cx : 0.0);
           }
         }
@@ -704,10 +701,11 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, bool m
   static bool attr_set = false;
   constexpr int kW = kDepTileWarps;
   auto kvec = k_deposit_tile<R, ORDER, kW>;
-  auto kmma = k_deposit_mma<R, ORDER, kW>;
+  auto kmma = k_deposit_mma<R, ORDER, kDepMmaWarps, kDepMmaCtas>;
+  constexpr int mw = kDepMmaWarps;
   const size_t push_smem = (size_t)6 * PushBox<ORDER>::VOL * sizeof(R);
   const size_t vec_smem = (size_t)kW * 32 * TWin<ORDER>::REC * sizeof(R);
-  const size_t mma_smem = (size_t)kW * 33 * MWin<ORDER>::REC * sizeof(R);
+  const size_t mma_smem = (size_t)mw * 33 * MWin<ORDER>::REC * sizeof(R);
   if (!attr_set) {
     cudaFuncSetAttribute(k_push_tile<R, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
     cudaFuncSetAttribute(kvec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vec_smem);
@@ -721,7 +719,7 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, bool m
   {
     ScopedPhase ph(c, kPhaseDeposit);
     if (mma)
-      kmma<<<n_tiles, kW * 32, mma_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
+      kmma<<<n_tiles, mw * 32, mma_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
                                                     a.stray_count, a.deactivated);
     else
       kvec<<<n_tiles, kW * 32, vec_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
