@@ -42,15 +42,53 @@ __global__ void __launch_bounds__(256) k_push_E(Grid<R> g, Box3 b) {
   g.F[2][t] += g.cE[0] * (by - By[t - 1]) - g.cE[1] * (bx - Bx[t - g.sy]) - g.cJ * g.J[2][t];
 }
 
+// The shell of thickness G of a box n0 x n1 x n2 (n >= 2G on every axis), enumerated without the
+// interior: 2G full z-planes, then 2G full y-rows of every other plane, then the 2G x-ends of every
+// other row. shell_size() points; shell_point() maps a running index to box coordinates.
+__host__ __device__ inline int64_t shell_size(int n0, int n1, int n2, int G) {
+  return (int64_t)2 * G * n0 * n1 + (int64_t)(n2 - 2 * G) * 2 * G * n0 + (int64_t)(n2 - 2 * G) * (n1 - 2 * G) * 2 * G;
+}
+__device__ __forceinline__ void shell_point(int64_t idx, int n0, int n1, int n2, int G, int& i, int& j, int& k) {
+  const int64_t nA = (int64_t)2 * G * n0 * n1, nB = (int64_t)(n2 - 2 * G) * 2 * G * n0;
+  if (idx < nA) {
+    i = (int)(idx % n0);
+    int64_t r = idx / n0;
+    j = (int)(r % n1);
+    int kk = (int)(r / n1);                    // 0 .. 2G-1
+    k = kk < G ? kk : n2 - 2 * G + kk;
+  } else if (idx < nA + nB) {
+    idx -= nA;
+    i = (int)(idx % n0);
+    int64_t r = idx / n0;
+    int jj = (int)(r % (2 * G));
+    j = jj < G ? jj : n1 - 2 * G + jj;
+    k = G + (int)(r / (2 * G));
+  } else {
+    idx -= nA + nB;
+    int ii = (int)(idx % (2 * G));
+    i = ii < G ? ii : n0 - 2 * G + ii;
+    int64_t r = idx / (2 * G);
+    j = G + (int)(r % (n1 - 2 * G));
+    k = G + (int)(r / (n1 - 2 * G));
+  }
+}
+
 // SumBoundary on one periodic box: every valid node within G of a periodic face collects its
 // guard images in a fixed order (deterministic, no atomics). Images on a non-periodic axis are
 // dropped. One thread per valid node of the shell; three components per thread.
-template <class R>
+template <class R, bool SHELL>
 __global__ void __launch_bounds__(256) k_fold_J(Grid<R> g) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  int j = blockIdx.y * blockDim.y + threadIdx.y;
-  int k = blockIdx.z;
-  if (i >= g.N[0] || j >= g.N[1]) return;
+  int i, j, k;
+  if constexpr (SHELL) {   // only the nodes within G of a face (needs N >= 2G)
+    const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= shell_size(g.N[0], g.N[1], g.N[2], kGuard)) return;
+    shell_point(idx, g.N[0], g.N[1], g.N[2], kGuard, i, j, k);
+  } else {
+    i = blockIdx.x * blockDim.x + threadIdx.x;
+    j = blockIdx.y * blockDim.y + threadIdx.y;
+    k = blockIdx.z;
+    if (i >= g.N[0] || j >= g.N[1]) return;
+  }
   const int G = kGuard;
   int c[3] = {i, j, k};
   int lo[3], hi[3];
@@ -83,10 +121,11 @@ struct ArrList { R* a[6]; int n; };
 
 template <class R>
 __global__ void __launch_bounds__(256) k_fill_guards(Grid<R> g, ArrList<R> arrs) {
-  int i = blockIdx.x * blockDim.x + threadIdx.x - kGuard;
-  int j = blockIdx.y * blockDim.y + threadIdx.y - kGuard;
-  int k = (int)blockIdx.z - kGuard;
-  if (i >= g.N[0] + kGuard || j >= g.N[1] + kGuard) return;
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;   // over the guard shell only
+  if (idx >= shell_size(g.P[0], g.P[1], g.P[2], kGuard)) return;
+  int i, j, k;
+  shell_point(idx, g.P[0], g.P[1], g.P[2], kGuard, i, j, k);
+  i -= kGuard; j -= kGuard; k -= kGuard;
   int c[3] = {i, j, k};
   int s[3];
   bool guard = false;
@@ -143,7 +182,12 @@ void launch_push_E(const Grid<R>& g, const int lo[3], const int hi[3], Ctx& c) {
 }
 template <class R>
 void launch_fold_J(const Grid<R>& g, Ctx& c) {
-  k_fold_J<R><<<grd(g.N[0], g.N[1], g.N[2]), blk(), 0, c.stream>>>(g);
+  if (g.N[0] >= 2 * kGuard && g.N[1] >= 2 * kGuard && g.N[2] >= 2 * kGuard) {
+    const int64_t n = shell_size(g.N[0], g.N[1], g.N[2], kGuard);
+    k_fold_J<R, true><<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(g);
+  } else {
+    k_fold_J<R, false><<<grd(g.N[0], g.N[1], g.N[2]), blk(), 0, c.stream>>>(g);
+  }
   c.launches++;
 }
 template <class R>
@@ -151,7 +195,8 @@ void launch_fill_guards(const Grid<R>& g, R* const* arrays, int narr, Ctx& c) {
   ArrList<R> l;
   l.n = narr;
   for (int a = 0; a < 6; ++a) l.a[a] = a < narr ? arrays[a] : nullptr;
-  k_fill_guards<R><<<grd(g.P[0], g.P[1], g.P[2]), blk(), 0, c.stream>>>(g, l);
+  const int64_t n = shell_size(g.P[0], g.P[1], g.P[2], kGuard);
+  k_fill_guards<R><<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(g, l);
   c.launches++;
 }
 template <class R>
