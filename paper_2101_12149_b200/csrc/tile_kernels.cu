@@ -462,8 +462,9 @@ __global__ void __launch_bounds__(NWARP * 32, 2)
 // The sums of one cell's particles are small dense contractions over the particles p:
 //   Jx[i][jk] += sum_p PX_p[i] * cx_p[jk]
 //   Jy[i][jk] += sum_p A_p[i] * (PY_p[j] S0z_p[k]) + B_p[i] * (PY_p[j] DSz_p[k])       (Jz alike)
-// with i the NX window nodes along x and jk the NYZ^2 columns, i.e. C[8 x 16] += A[8 x K] B[K x 16],
-// K = particles (Jx) or 2 x particles (Jy, Jz): mma.sync.m8n8k4.f64 (DMMA), one warp per cell batch.
+// with i the NX window nodes along x and jk the NYZ^2 columns, i.e. C[8 x 16] += A[8 x K] B[K x 16]
+// with K = particles, four per step (Jy and Jz take two steps each, one per term):
+// mma.sync.m8n8k4.f64 (DMMA), ten per four particles, one warp per run of same-cell particles.
 // Row r of C holds window node X with X mod 8 == r, so C never moves when the window advances: the
 // row of the node that left is reduced into J (one RED per element) and reused.
 __device__ __forceinline__ void dmma_884(double& c0, double& c1, double a, double b) {
@@ -515,7 +516,6 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int gq = lane >> 2, t = lane & 3;           // fragment coordinates of this lane
-  const int term = t & 1;
   R* rec = rec_all + (size_t)warp * 33 * REC;       // 32 records of the round + one that stays zero
   const R* zrec = rec + 32 * REC;
   for (int i = lane; i < REC; i += 32) rec[32 * REC + i] = R(0);
@@ -634,36 +634,29 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
       }
       const int i = (gq - win_x(cd)) & 7;          // window slot of this lane's row
       const bool rowok = i < NX;
-      const int offPX = W::oPX + (rowok ? i : 0), offAB = W::oAB + 2 * (rowok ? i : 0) + term;
+      const int offPX = W::oPX + (rowok ? i : 0), offAB = W::oAB + 2 * (rowok ? i : 0);
 #pragma unroll 2
       for (int b = s0; b < s1; b += 4) {
-        {   // Jx: four particles, K = particle
-          const R* rr = rec + (b + t < s1 ? b + t : 32) * REC;      // slot 32: the all-zero record
-          const R* ra = rowok ? rr : zrec;
-          const double a = ra[offPX];
-          const Pair2<R> yv = *reinterpret_cast<const Pair2<R>*>(rr + offY);
-          const double al = fma(0.5, (double)yv.b, (double)yv.a), be = fma(0.5, (double)yv.a, (double)yv.b * (1.0 / 3.0));
+        // four particles per contraction step, K = particle: this lane supplies, for particle b + t,
+        // the A operands of its row (window node) and the B operands of its column(s)
+        const R* rr = rec + (b + t < s1 ? b + t : 32) * REC;      // slot 32: the all-zero record
+        const R* ra = rowok ? rr : zrec;
+        const double px = ra[offPX];
+        const Pair2<R> ab = *reinterpret_cast<const Pair2<R>*>(ra + offAB);
+        const Pair2<R> yv = *reinterpret_cast<const Pair2<R>*>(rr + offY);
+        const double py = colok ? (double)rr[offPY] : 0.0;
+        const double y0 = colok ? (double)yv.a : 0.0, y1 = colok ? (double)yv.b : 0.0;
+        const double al = fma(0.5, y1, y0), be = fma(0.5, y0, y1 * (1.0 / 3.0));
 #pragma unroll
-          for (int nb = 0; nb < NB; ++nb) {
-            const Pair2<R> zv = *reinterpret_cast<const Pair2<R>*>(rr + offZ + 2 * W::KSTEP * nb);
-            const double cx = fma((double)zv.a, al, (double)zv.b * be);
-            dmma_884(C.x[nb][0], C.x[nb][1], a, colok ? cx : 0.0);
-          }
-        }
-#pragma unroll
-        for (int q = 0; q < 2; ++q) {   // Jy, Jz: two particles each, K = (particle, term)
-          if (q == 1 && b + 2 >= s1) break;
-          const int idx = b + 2 * q + (t >> 1);
-          const R* rr = rec + (idx < s1 ? idx : 32) * REC;
-          const R* ra = rowok ? rr : zrec;
-          const double a = ra[offAB];
-          const double yel = rr[offY + term], py = rr[offPY];
-#pragma unroll
-          for (int nb = 0; nb < NB; ++nb) {
-            const double zel = rr[offZ + 2 * W::KSTEP * nb + term], pz = rr[offPZ + W::KSTEP * nb];
-            dmma_884(C.y[nb][0], C.y[nb][1], a, colok ? py * zel : 0.0);
-            dmma_884(C.z[nb][0], C.z[nb][1], a, colok ? pz * yel : 0.0);
-          }
+        for (int nb = 0; nb < NB; ++nb) {
+          const Pair2<R> zv = *reinterpret_cast<const Pair2<R>*>(rr + offZ + 2 * W::KSTEP * nb);
+          const double pz = rr[offPZ + W::KSTEP * nb];
+          const double z0 = zv.a, z1 = zv.b;
+          dmma_884(C.x[nb][0], C.x[nb][1], px, fma(z0, al, z1 * be));
+          dmma_884(C.y[nb][0], C.y[nb][1], (double)ab.a, py * z0);
+          dmma_884(C.z[nb][0], C.z[nb][1], (double)ab.a, pz * y0);
+          dmma_884(C.y[nb][0], C.y[nb][1], (double)ab.b, py * z1);
+          dmma_884(C.z[nb][0], C.z[nb][1], (double)ab.b, pz * y1);
         }
       }
     }
