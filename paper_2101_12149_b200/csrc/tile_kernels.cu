@@ -540,18 +540,18 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
 
   CFrag<NB> C;
   C.zero();
-  int cur = INT_MIN;   // packed cell of the window being accumulated
-  auto win_x = [&](int cd) { return tb[0] + (cd & 15) - 4 - BLX; };
+  int cur = INT_MIN;   // packed cell triple of the window being accumulated
+  auto win_x = [&](int cd) { return tb[0] + 3 * (cd & 15) - 4 - BLX; };   // first node of a triple's 8-node window
   auto win_y = [&](int cd) { return tb[1] + ((cd >> 4) & 15) - 4 - BLYZ; };
   auto win_z = [&](int cd) { return tb[2] + (cd >> 8) - 4 - BLYZ; };
-  // rows of the old window that the new one (nx0 .. nx0+NX-1 on the same y,z; none if !same_row) does
+  // rows of the old window that the new one (nx0 .. nx0+7 on the same y,z; none if !same_row) does
   // not contain go to J, one reduction per element, and are cleared
   auto retire_rows = [&](bool same_row, int nx0) {
     const int ox0 = win_x(cur);
     const int io = (gq - ox0) & 7;
     const int X = ox0 + io;
-    const bool keep = same_row && X >= nx0 && X < nx0 + NX;
-    if (io < NX && !keep) {
+    const bool keep = same_row && X >= nx0 && X < nx0 + 8;
+    if (!keep) {
       const int base = g.idx(X, win_y(cur), win_z(cur));
 #pragma unroll
       for (int b = 0; b < NB; ++b)
@@ -617,32 +617,38 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
       }
     }
     __syncwarp();
-    // runs of consecutive particles with the same window (the order is cell-sorted up to drift since
-    // the last sort; a cell met twice is simply accumulated twice). Warp-uniform control flow.
-    const int prev = __shfl_up_sync(0xffffffffu, code, 1);
-    unsigned heads = __ballot_sync(0xffffffffu, lane == 0 || code != prev);
+    // runs of consecutive particles whose cells lie in the same triple of x-neighbouring cells of one
+    // (y,z) row: their windows span 8 nodes together, exactly the 8 rows of C, so they share the
+    // accumulators (fewer padded contraction steps, and three rows retire at once). The order is
+    // cell-sorted up to drift since the last sort; a triple met twice is simply accumulated twice.
+    // Warp-uniform control flow.
+    const int scode = code < 0 ? -1 : ((code & ~15) | ((code & 15) / 3));
+    const int prev = __shfl_up_sync(0xffffffffu, scode, 1);
+    unsigned heads = __ballot_sync(0xffffffffu, lane == 0 || scode != prev);
     const unsigned live = __ballot_sync(0xffffffffu, code >= 0);
     while (heads) {
       const int s0 = __ffs(heads) - 1;
       heads &= heads - 1;
       const int s1 = heads ? __ffs(heads) - 1 : 32;
       if (!((live >> s0) & 1u)) continue;
-      const int cd = __shfl_sync(0xffffffffu, code, s0);
+      const int cd = __shfl_sync(0xffffffffu, scode, s0);
       if (cd != cur) {
         if (cur != INT_MIN) retire_rows(((cd ^ cur) >> 4) == 0, win_x(cd));
         cur = cd;
       }
-      const int i = (gq - win_x(cd)) & 7;          // window slot of this lane's row
-      const bool rowok = i < NX;
-      const int offPX = W::oPX + (rowok ? i : 0), offAB = W::oAB + 2 * (rowok ? i : 0);
 #pragma unroll 2
       for (int b = s0; b < s1; b += 4) {
         // four particles per contraction step, K = particle: this lane supplies, for particle b + t,
-        // the A operands of its row (window node) and the B operands of its column(s)
-        const R* rr = rec + (b + t < s1 ? b + t : 32) * REC;      // slot 32: the all-zero record
+        // the A operands of its row (a node of that particle's own 6-node window, or zero) and the
+        // B operands of its column(s)
+        const bool here = b + t < s1;
+        const int pc = __shfl_sync(0xffffffffu, code, (b + t) & 31);
+        const int i = (gq - (tb[0] + (pc & 15) - 4 - BLX)) & 7;      // window slot of this lane's row
+        const bool rowok = i < NX;
+        const R* rr = rec + (here ? b + t : 32) * REC;               // slot 32: the all-zero record
         const R* ra = rowok ? rr : zrec;
-        const double px = ra[offPX];
-        const Pair2<R> ab = *reinterpret_cast<const Pair2<R>*>(ra + offAB);
+        const double px = ra[W::oPX + (rowok ? i : 0)];
+        const Pair2<R> ab = *reinterpret_cast<const Pair2<R>*>(ra + W::oAB + 2 * (rowok ? i : 0));
         const Pair2<R> yv = *reinterpret_cast<const Pair2<R>*>(rr + offY);
         const double py = colok ? (double)rr[offPY] : 0.0;
         const double y0 = colok ? (double)yv.a : 0.0, y1 = colok ? (double)yv.b : 0.0;
