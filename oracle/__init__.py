@@ -57,6 +57,10 @@ def lib():
         L.orc_particle_step.argtypes = [vp]
         L.orc_shape_f64.argtypes = [C.c_int, C.c_double, i32p, dp]
         L.orc_shape_f32.argtypes = [C.c_int, C.c_float, i32p, C.POINTER(C.c_float)]
+        L.orc_set_method.argtypes = [vp, C.c_int, C.c_int]
+        L.orc_set_method.restype = C.c_int
+        L.orc_vay_f64.argtypes = [C.c_double, dp, dp, dp]
+        L.orc_vay_f32.argtypes = [C.c_float] + [C.POINTER(C.c_float)] * 3
         L.orc_boris_f64.argtypes = [C.c_double, dp, dp, dp]
         L.orc_boris_f32.argtypes = [C.c_float] + [C.POINTER(C.c_float)] * 3
         L.orc_gather.argtypes = [vp, C.c_int64, vp, vp, vp, vp]
@@ -98,11 +102,26 @@ def boris(kq: float, E, B, u, dtype=np.float64):
     return u
 
 
+def vay(kq: float, E, B, u, dtype=np.float64):
+    """One Vay push u^{n-1/2} -> u^{n+1/2} (ref [21]). kq = q*dt/(2m)."""
+    E = np.ascontiguousarray(E, dtype=dtype)
+    B = np.ascontiguousarray(B, dtype=dtype)
+    u = np.array(u, dtype=dtype)
+    ct = C.c_double if np.dtype(dtype) == np.float64 else C.c_float
+    f = lib().orc_vay_f64 if np.dtype(dtype) == np.float64 else lib().orc_vay_f32
+    f(ct(kq), E.ctypes.data_as(C.POINTER(ct)), B.ctypes.data_as(C.POINTER(ct)), u.ctypes.data_as(C.POINTER(ct)))
+    return u
+
+
+PUSHER_BORIS, PUSHER_VAY = 0, 1
+GATHER_UNIFORM, GATHER_GALERKIN = 0, 1
+
+
 class Oracle:
     """One oracle simulation. Arrays in and out are numpy, x-fastest fields of shape (nz, ny, nx)."""
 
     def __init__(self, n_cells, dx, dt, order, dtype=np.float64, periodic=(1, 1, 1), tile=(8, 8, 8),
-                 sort_interval=4, sort_key_mode=0):
+                 sort_interval=4, sort_key_mode=0, pusher=PUSHER_BORIS, gather_mode=GATHER_UNIFORM):
         self.dtype = np.dtype(dtype)
         self.n_cells = tuple(int(v) for v in n_cells)
         self.dx = tuple(float(v) for v in dx)
@@ -116,6 +135,8 @@ class Oracle:
         if not self._h:
             raise ValueError("orc_create rejected the arguments (order, tile, dx or CFL)")
         self._fshape = (self.n_cells[2], self.n_cells[1], self.n_cells[0])
+        if lib().orc_set_method(self._h, int(pusher), int(gather_mode)) != 0:
+            raise ValueError("unknown pusher / gather_mode")
 
     def close(self):
         if self._h:

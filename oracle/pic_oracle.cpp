@@ -49,7 +49,11 @@ const double kStag[6][3] = {
 // n+1 weights (B-splines of order 1..3).
 template <class R>
 void shape(int n, R xi, int* l, R* w) {
-  if (n == 1) {
+  if (n == 0) {                         // nearest grid point (only the Galerkin gather at order 1 uses it)
+    R m = std::floor(xi + R(0.5));
+    *l = (int)m;
+    w[0] = R(1);
+  } else if (n == 1) {
     R m = std::floor(xi);
     R d = xi - m;
     *l = (int)m;
@@ -92,6 +96,8 @@ struct Sim {
   int periodic[3];
   int tile[3];
   int sort_interval, key_mode;
+  int pusher = 0;        // 0 Boris (reading Q2), 1 Vay (ref [21])
+  int gather_mode = 0;   // 0 uniform order (reading Q1), 1 Galerkin / energy-conserving (NEXT-2)
   // coefficient block (C-list): computed in double, rounded once to R
   R inv_dx[3], L[3], cB[3], cE[3], cJ, inv_c2, dtr;
   std::vector<R> F[6];        // Ex,Ey,Ez,Bx,By,Bz ; x fastest
@@ -134,14 +140,19 @@ R gather(const Sim<R>& s, int comp, R x, R y, R z) {
   int l[3];
   R w[3][4];
   R pos[3] = {x, y, z};
+  // Galerkin ("energy-conserving") variant: order n-1 along every axis on which the component is
+  // staggered, order n along the others (it is the gather whose weights equal the
+  // Esirkepov deposit's in the limit of a small move, see pin T14)
+  int nd[3];
   for (int d = 0; d < 3; ++d) {
+    nd[d] = (s.gather_mode == 1 && kStag[comp][d] != 0.0) ? n - 1 : n;
     R xi = pos[d] * s.inv_dx[d] - R(kStag[comp][d]);
-    shape<R>(n, xi, &l[d], w[d]);
+    shape<R>(nd[d], xi, &l[d], w[d]);
   }
   R acc = 0;
-  for (int c = 0; c <= n; ++c)
-    for (int b = 0; b <= n; ++b)
-      for (int a = 0; a <= n; ++a)
+  for (int c = 0; c <= nd[2]; ++c)
+    for (int b = 0; b <= nd[1]; ++b)
+      for (int a = 0; a <= nd[0]; ++a)
         acc += w[0][a] * w[1][b] * w[2][c] * s.rd(s.F[comp], l[0] + a, l[1] + b, l[2] + c);
   return acc;
 }
@@ -163,6 +174,34 @@ void boris(R kq, R inv_c2, const R E[3], const R B[3], R u[3]) {
   upl[1] = um[1] + (up[2] * sv[0] - up[0] * sv[2]);
   upl[2] = um[2] + (up[0] * sv[1] - up[1] * sv[0]);
   for (int d = 0; d < 3; ++d) u[d] = upl[d] + kq * E[d];
+}
+
+// Vay pusher ("Vay pusher", ref [21] = J.-L. Vay, Phys. Plasmas 15, 056701 (2008));
+// u = gamma*v in m/s, kq = q*dt/(2m), in the paper's order:
+//   u' = u + 2 kq E + kq (u/gamma) x B;  tau = kq B;  u* = u'.tau / c;  gamma' = sqrt(1 + u'^2/c^2)
+//   sigma = gamma'^2 - tau^2;  gamma_new = sqrt((sigma + sqrt(sigma^2 + 4 (tau^2 + u*^2))) / 2)
+//   t = tau / gamma_new;  u_new = (u' + (u'.t) t + u' x t) / (1 + t^2)
+template <class R>
+void vay(R kq, R inv_c2, const R E[3], const R B[3], R u[3]) {
+  R g0 = std::sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * inv_c2);
+  R v[3] = {u[0] / g0, u[1] / g0, u[2] / g0};
+  R up[3], tau[3], t[3];
+  up[0] = u[0] + R(2) * kq * E[0] + kq * (v[1] * B[2] - v[2] * B[1]);
+  up[1] = u[1] + R(2) * kq * E[1] + kq * (v[2] * B[0] - v[0] * B[2]);
+  up[2] = u[2] + R(2) * kq * E[2] + kq * (v[0] * B[1] - v[1] * B[0]);
+  for (int d = 0; d < 3; ++d) tau[d] = kq * B[d];
+  R tau2 = tau[0] * tau[0] + tau[1] * tau[1] + tau[2] * tau[2];
+  R us = (up[0] * tau[0] + up[1] * tau[1] + up[2] * tau[2]) * std::sqrt(inv_c2);
+  R gp2 = R(1) + (up[0] * up[0] + up[1] * up[1] + up[2] * up[2]) * inv_c2;
+  R sigma = gp2 - tau2;
+  R gn = std::sqrt((sigma + std::sqrt(sigma * sigma + R(4) * (tau2 + us * us))) / R(2));
+  for (int d = 0; d < 3; ++d) t[d] = tau[d] / gn;
+  R t2 = t[0] * t[0] + t[1] * t[1] + t[2] * t[2];
+  R ut = up[0] * t[0] + up[1] * t[1] + up[2] * t[2];
+  R sc = R(1) / (R(1) + t2);
+  u[0] = sc * (up[0] + ut * t[0] + (up[1] * t[2] - up[2] * t[1]));
+  u[1] = sc * (up[1] + ut * t[1] + (up[2] * t[0] - up[0] * t[2]));
+  u[2] = sc * (up[2] + ut * t[2] + (up[0] * t[1] - up[1] * t[0]));
 }
 
 // ---------------------------------------------------------------- step 2e
@@ -317,7 +356,8 @@ void particles_step(Sim<R>& s) {
         E[c] = gather<R>(s, c, x0[0], x0[1], x0[2]);
         B[c] = gather<R>(s, 3 + c, x0[0], x0[1], x0[2]);
       }
-      boris<R>(sp.kq, s.inv_c2, E, B, u);                  // 2c
+      if (s.pusher == 1) vay<R>(sp.kq, s.inv_c2, E, B, u);
+      else boris<R>(sp.kq, s.inv_c2, E, B, u);             // 2c
       R g = std::sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * s.inv_c2);
       R x1[3];
       for (int d = 0; d < 3; ++d) x1[d] = x0[d] + s.dtr * u[d] / g;   // 2d (unwrapped)
@@ -619,6 +659,20 @@ void orc_particle_step(void* hv) {
 
 void orc_shape_f64(int order, double xi, int32_t* l, double* w) { int ll; shape<double>(order, xi, &ll, w); *l = ll; }
 void orc_shape_f32(int order, float xi, int32_t* l, float* w) { int ll; shape<float>(order, xi, &ll, w); *l = ll; }
+// pusher: 0 Boris, 1 Vay; gather_mode: 0 uniform order, 1 Galerkin. Returns 0, or -1 for bad values.
+int orc_set_method(void* hv, int pusher, int gather_mode) {
+  auto* h = (Handle*)hv;
+  if (!h || pusher < 0 || pusher > 1 || gather_mode < 0 || gather_mode > 1) return -1;
+  if (h->prec == 0) { h->d->pusher = pusher; h->d->gather_mode = gather_mode; }
+  else { h->f->pusher = pusher; h->f->gather_mode = gather_mode; }
+  return 0;
+}
+void orc_vay_f64(double kq, const double* E, const double* B, double* u) {
+  vay<double>(kq, 1.0 / (kC * kC), E, B, u);
+}
+void orc_vay_f32(float kq, const float* E, const float* B, float* u) {
+  vay<float>(kq, (float)(1.0 / (kC * kC)), E, B, u);
+}
 void orc_boris_f64(double kq, const double* E, const double* B, double* u) {
   boris<double>(kq, 1.0 / (kC * kC), E, B, u);
 }

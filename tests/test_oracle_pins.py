@@ -519,3 +519,155 @@ def test_nonperiodic_axis_reads_zero_and_drops_writes():
         assert np.array_equal(Jn[d][:5], Jp[d][:5])
         assert np.all(Jn[d][5:] == 0)
     assert any(np.any(Jp[d][5:] != 0) for d in range(3))
+
+
+# --------------------------------------------------------------------------- T13 Vay pusher (NEXT-4)
+def test_T13_vay_keeps_the_ExB_drift_exactly_and_boris_does_not():
+    """Defining property of the Vay pusher (ref [21]): a particle that moves with the
+    drift velocity v = E x B / B^2 (E perpendicular to B, E < cB) feels no net force, at any gamma and any
+    time step; the Boris rotation leaves a spurious force of order (omega_c dt)^2."""
+    rng = np.random.default_rng(130)
+    for _ in range(50):
+        B = rng.normal(size=3)
+        Bn = np.linalg.norm(B)
+        e = np.cross(B, rng.normal(size=3))
+        e /= np.linalg.norm(e)
+        beta = rng.uniform(0.05, 0.98)
+        E = beta * c * Bn * e                      # |E| = beta c |B|, perpendicular to B
+        vd = np.cross(E, B) / Bn ** 2
+        assert abs(np.linalg.norm(vd) / c - beta) < 1e-12
+        u0 = vd / math.sqrt(1 - beta * beta)
+        kq = rng.uniform(0.05, 1.5) / Bn * rng.choice([-1.0, 1.0])     # |omega_c dt / 2| up to 1.5
+        uv = oracle.vay(kq, E, B, u0)
+        assert np.linalg.norm(uv - u0) < 1e-13 * np.linalg.norm(u0)
+        ub = oracle.boris(kq, E, B, u0)
+        if beta > 0.5 and abs(kq) * Bn > 0.3:
+            assert np.linalg.norm(ub - u0) > 1e-4 * np.linalg.norm(u0)
+
+
+def test_T13_vay_limits_pure_E_pure_B_and_agreement_with_boris():
+    rng = np.random.default_rng(131)
+    for _ in range(30):
+        u0 = rng.normal(size=3) * c * rng.uniform(0.01, 3.0)
+        E = rng.normal(size=3) * 1e9
+        B = rng.normal(size=3)
+        kq = rng.uniform(-1.0, 1.0) * 1e-1
+        # B = 0: u += 2 kq E exactly, as for Boris
+        assert np.allclose(oracle.vay(kq, E, 0 * B, u0), u0 + 2 * kq * E, rtol=1e-15, atol=0)
+        # E = 0: |u| is conserved (gamma_new = gamma, shown in closed form in DESIGN.md)
+        assert abs(np.linalg.norm(oracle.vay(kq, 0 * E, B, u0)) / np.linalg.norm(u0) - 1) < 1e-14
+    # both pushers are second order: their difference shrinks as dt^3 per step
+    u0 = np.array([0.3, -0.2, 0.5]) * c
+    E = np.array([1.0, 2.0, -1.5]) * 1e10
+    B = np.array([0.5, -1.0, 2.0])
+    d = [np.linalg.norm(oracle.vay(kq, E, B, u0) - oracle.boris(kq, E, B, u0)) for kq in (-5e-4, -2.5e-4, -1.25e-4)]
+    assert 7.0 < d[0] / d[1] < 10.0 and 7.0 < d[1] / d[2] < 10.0 and d[1] / d[2] < d[0] / d[1]
+
+
+def test_T13_vay_gyration_conserves_energy_and_closes_the_orbit():
+    """Uniform B through the whole oracle loop with pusher = Vay: |u| stays constant to roundoff and
+    the rotation per step is the same 2 atan(omega_c dt / 2) as Boris (for E = 0 the two coincide:
+    u' = u + u x t, then the same normalisation)."""
+    n, dx = (8, 8, 8), (1e-6, 1e-6, 1e-6)
+    dt = 0.5 * dx[0] / (c * math.sqrt(3))
+    B0 = 2.0e3
+    o = Oracle(n, dx, dt, 1, sort_interval=0, pusher=oracle.PUSHER_VAY)
+    Bz = np.full((8, 8, 8), B0)
+    zf = np.zeros((8, 8, 8))
+    o.set_fields([zf, zf, zf], [zf, zf, Bz])
+    u0 = 0.5 * c
+    o.add_species([4e-6], [4e-6], [4e-6], [u0], [0.0], [0.0], [0.0], -Q_E, M_E)      # weight 0: no J
+    gam = math.sqrt(1 + (u0 / c) ** 2)
+    wc = Q_E * B0 / (gam * M_E)
+    theta = 2 * math.atan(wc * dt / 2)
+    ang = []
+    for _ in range(40):
+        o.step(1)
+        p = o.get_particles(0)
+        assert abs(math.hypot(p["ux"][0], p["uy"][0]) / u0 - 1) < 1e-13
+        ang.append(math.atan2(p["uy"][0], p["ux"][0]))
+    dth = np.diff(np.unwrap(ang))
+    assert np.all(dth > 0)                         # electron, B along +z: counter-clockwise
+    assert np.max(np.abs(dth - theta)) < 1e-12
+
+
+# --------------------------------------------------------------------------- T14 Galerkin gather (NEXT-2)
+_STAG = [(1, 0, 0), (0, 1, 0), (0, 0, 1), (0, 1, 1), (1, 0, 1), (1, 1, 0)]   # Ex Ey Ez Bx By Bz
+
+
+def _cardinal_bspline(m, d):
+    """Centred cardinal B-spline of degree m at distance d, from scipy's B-spline basis (an
+    implementation that shares nothing with oracle.shape)."""
+    from scipy.interpolate import BSpline
+    knots = np.arange(m + 2) - (m + 1) / 2.0
+    b = BSpline.basis_element(knots, extrapolate=False)
+    v = b(d)
+    return 0.0 if np.isnan(v) else float(v)
+
+
+@pytest.mark.parametrize("order", [1, 2, 3])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_T14_gather_equals_the_tensor_product_of_library_bsplines(order, mode):
+    """Both gather variants against a dense sum over ALL nodes of a small periodic grid with 1-D
+    weights from scipy.interpolate.BSpline: degree n on every axis (uniform), or n-1 along the axes on
+    which the component is staggered (Galerkin). Fixes offsets, orders and indices."""
+    n, dx = (6, 5, 7), (1.0e-6, 0.8e-6, 0.5e-6)
+    dt = 0.5 / (c * math.sqrt(sum(1 / d ** 2 for d in dx)))
+    rng = np.random.default_rng(140 + order)
+    o = Oracle(n, dx, dt, order, sort_interval=0, gather_mode=mode)
+    F = [rng.normal(size=(n[2], n[1], n[0])) for _ in range(6)]
+    o.set_fields(F[:3], F[3:])
+    npart = 12
+    pos = rng.uniform(0, 1, size=(npart, 3)) * np.array(n) * np.array(dx)
+    got = o.gather(pos[:, 0], pos[:, 1], pos[:, 2])
+    for p in range(npart):
+        for comp in range(6):
+            W = []
+            for d in range(3):
+                deg = order - 1 if (mode == 1 and _STAG[comp][d]) else order
+                xi = pos[p, d] / dx[d] - 0.5 * _STAG[comp][d]
+                w = np.zeros(n[d])
+                for i in range(-4, n[d] + 4):          # periodic images
+                    if deg == 0:
+                        w[i % n[d]] += 1.0 if -0.5 <= xi - i < 0.5 else 0.0
+                    else:
+                        w[i % n[d]] += _cardinal_bspline(deg, xi - i)
+                W.append(w)
+            want = np.einsum("kji,k,j,i->", F[comp], W[2], W[1], W[0])
+            assert abs(got[p, comp] - want) < 1e-13 * (1 + abs(want)), (p, comp)
+
+
+@pytest.mark.parametrize("order", [1, 2, 3])
+def test_T14_galerkin_gather_is_the_small_move_limit_of_the_esirkepov_deposit(order):
+    """Energy exchange identity that gives the variant its name: for a move delta along one axis, the
+    work of the field on the deposited current, sum_nodes J_d E_d dV dt, equals q w delta E_d gathered at
+    the midpoint with the Galerkin weights, up to O(delta^2) (d/dx of a degree-n B-spline is the
+    difference of two degree n-1 ones at the staggered points). The deposit is pinned by T5-T7."""
+    n, dx = (7, 6, 8), (1.0e-6, 0.8e-6, 0.5e-6)
+    dt = 0.5 / (c * math.sqrt(sum(1 / d ** 2 for d in dx)))
+    rng = np.random.default_rng(150 + order)
+    E = [rng.normal(size=(n[2], n[1], n[0])) for _ in range(3)]
+    zf = np.zeros((n[2], n[1], n[0]))
+    og = Oracle(n, dx, dt, order, sort_interval=0, gather_mode=1)
+    ou = Oracle(n, dx, dt, order, sort_interval=0, gather_mode=0)
+    for o in (og, ou):
+        o.set_fields(E, [zf, zf, zf])
+        o.add_species([0.], [0.], [0.], [0.], [0.], [0.], [1.], -Q_E, M_E)
+    dv = dx[0] * dx[1] * dx[2]
+    w = np.array([2.5e5])
+    worst_uniform = 0.0
+    for trial in range(12):
+        d = trial % 3
+        xm = rng.uniform(0.2, 0.8, 3) * np.array(n) * np.array(dx)
+        delta = 1e-4 * dx[d]
+        x0, x1 = xm.copy(), xm.copy()
+        x0[d] -= delta / 2
+        x1[d] += delta / 2
+        J = og.deposit_moves(0, x0[None, :], x1[None, :], w)
+        work = float(np.sum(J[d] * E[d])) * dv * dt
+        eg = og.gather([xm[0]], [xm[1]], [xm[2]])[0, d]
+        eu = ou.gather([xm[0]], [xm[1]], [xm[2]])[0, d]
+        scale = Q_E * w[0] * delta * np.max(np.abs(E[d]))
+        assert abs(work - (-Q_E) * w[0] * delta * eg) < 1e-6 * scale
+        worst_uniform = max(worst_uniform, abs(work - (-Q_E) * w[0] * delta * eu) / scale)
+    assert worst_uniform > 1e-3          # the uniform-order gather does NOT satisfy it: the pin discriminates
