@@ -79,6 +79,16 @@ enum {
                                  one warp per cell run. AUTO picks this in fp64 when it can. */
 };
 
+/* Momentum update of step 2c. BORIS: the relativistic Boris rotation (BASELINE.json; DESIGN.md
+ * reading Q2). VAY: the Vay pusher the paper's LWFA run uses (ref [21]; SURVEY.md
+ * 8(f) NEXT-4): u' = u + 2 kq E + kq (u/gamma) x B, then the closed-form gamma and rotation. */
+enum { PIC_PUSHER_BORIS = 0, PIC_PUSHER_VAY = 1 };
+
+/* Field gather of step 2b. UNIFORM: order n on every axis, each component from its own staggered
+ * location (reading Q1). GALERKIN: order n-1 along every axis on which the component is
+ * staggered ("energy-conserving" gather). */
+enum { PIC_GATHER_UNIFORM = 0, PIC_GATHER_GALERKIN = 1 };
+
 /* Options; pass NULL to pic_create for the defaults given here. */
 typedef struct {
   int32_t periodic[3];   /* default {1,1,1}; 0 = truncation with zeroed guard cells on that axis:
@@ -91,6 +101,8 @@ typedef struct {
   int32_t sort_key_mode; /* 0 = tile-major cell key (default): tile index major, cell inside
                             the tile minor; 1 = tile index only */
   int32_t deposit_mode;  /* PIC_DEPOSIT_*; default PIC_DEPOSIT_AUTO */
+  int32_t pusher;        /* PIC_PUSHER_*; default PIC_PUSHER_BORIS */
+  int32_t gather_mode;   /* PIC_GATHER_*; default PIC_GATHER_UNIFORM */
   int32_t reserved;      /* must be 0 */
   void*   cuda_stream;   /* cudaStream_t all work is issued on (e.g. torch's current stream);
                             NULL = the legacy default stream */

@@ -19,6 +19,8 @@ struct Grid {
   int sy, sz;        // strides of j and k in elements (sx = 1)
   int org;           // linear offset of node (0,0,0)
   int periodic[3];
+  int pusher;        // PIC_PUSHER_*
+  int gather_mode;   // PIC_GATHER_*
   R inv_dx[3], L[3], cB[3], cE[3], cJ, inv_c2, dt;
   R* F[6];           // Ex Ey Ez Bx By Bz
   R* J[3];
@@ -71,6 +73,19 @@ __device__ __forceinline__ int shape(R xi, R* w) {
     w[2] = (R(4) - R(6) * e * e + R(3) * e * e * e) * s;
     w[3] = d * d * d * s;
     return (int)m - 1;
+  }
+}
+
+// Galerkin gather: order ORDER-1 at a staggered coordinate, returned on ORDER+1 slots
+// (the last weight is zero) so that it drops into the loops of the uniform gather unchanged.
+template <class R, int ORDER>
+__device__ __forceinline__ int shape_lowered(R xi, R* w) {
+  w[ORDER] = R(0);
+  if constexpr (ORDER == 1) {            // order 0: nearest grid point
+    w[0] = R(1);
+    return (int)floor(xi + R(0.5));
+  } else {
+    return shape<R, ORDER - 1>(xi, w);
   }
 }
 

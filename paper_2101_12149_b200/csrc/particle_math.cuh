@@ -27,7 +27,7 @@ __device__ __forceinline__ R interp(const R* __restrict__ F, int base, int sy, i
   return acc;
 }
 
-template <class R, int ORDER>
+template <class R, int ORDER, bool GENERIC = true>
 __device__ __forceinline__ void gather6(const Grid<R>& g, R x, R y, R z, R* E, R* B) {
   // nodal (offset 0) and staggered (offset 1/2) weight sets per axis, shared by the components
   R wn[3][ORDER + 1], ws[3][ORDER + 1];
@@ -37,7 +37,8 @@ __device__ __forceinline__ void gather6(const Grid<R>& g, R x, R y, R z, R* E, R
   for (int d = 0; d < 3; ++d) {
     R xi = pos[d] * g.inv_dx[d];
     ln[d] = shape<R, ORDER>(xi, wn[d]);
-    ls[d] = shape<R, ORDER>(xi - R(0.5), ws[d]);
+    ls[d] = (GENERIC && g.gather_mode) ? shape_lowered<R, ORDER>(xi - R(0.5), ws[d])
+                                       : shape<R, ORDER>(xi - R(0.5), ws[d]);
     // memory safety if a position ever went non-finite: keep the stencil inside the padded box
     ln[d] = min(max(ln[d], -kGuard), g.N[d] + kGuard - ORDER - 1);
     ls[d] = min(max(ls[d], -kGuard), g.N[d] + kGuard - ORDER - 1);
@@ -66,6 +67,38 @@ __device__ __forceinline__ void boris(R kq, R inv_c2, const R* E, const R* B, R*
   u[0] = um0 + (up1 * s2 - up2 * s1) + kq * E[0];
   u[1] = um1 + (up2 * s0 - up0 * s2) + kq * E[1];
   u[2] = um2 + (up0 * s1 - up1 * s0) + kq * E[2];
+}
+
+// ------------------------------------------------------------------ Vay (ref [21])
+// u' = u + 2 kq E + kq (u/gamma) x B; tau = kq B; u* = u'.tau/c; sigma = gamma'^2 - tau^2;
+// gamma_new = sqrt((sigma + sqrt(sigma^2 + 4 (tau^2 + u*^2))) / 2); t = tau/gamma_new;
+// u_new = (u' + (u'.t) t + u' x t) / (1 + t^2)
+template <class R>
+__device__ __forceinline__ void vay(R kq, R inv_c2, const R* E, const R* B, R* u) {
+  const R ig0 = R(1) / sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * inv_c2);
+  const R v0 = u[0] * ig0, v1 = u[1] * ig0, v2 = u[2] * ig0;
+  const R up0 = u[0] + R(2) * kq * E[0] + kq * (v1 * B[2] - v2 * B[1]);
+  const R up1 = u[1] + R(2) * kq * E[1] + kq * (v2 * B[0] - v0 * B[2]);
+  const R up2 = u[2] + R(2) * kq * E[2] + kq * (v0 * B[1] - v1 * B[0]);
+  const R ta0 = kq * B[0], ta1 = kq * B[1], ta2 = kq * B[2];
+  const R tau2 = ta0 * ta0 + ta1 * ta1 + ta2 * ta2;
+  const R us = (up0 * ta0 + up1 * ta1 + up2 * ta2) * sqrt(inv_c2);
+  const R gp2 = R(1) + (up0 * up0 + up1 * up1 + up2 * up2) * inv_c2;
+  const R sigma = gp2 - tau2;
+  const R ign = R(1) / sqrt((sigma + sqrt(sigma * sigma + R(4) * (tau2 + us * us))) * R(0.5));
+  const R t0 = ta0 * ign, t1 = ta1 * ign, t2 = ta2 * ign;
+  const R ut = up0 * t0 + up1 * t1 + up2 * t2;
+  const R sc = R(1) / (R(1) + (t0 * t0 + t1 * t1 + t2 * t2));
+  u[0] = sc * (up0 + ut * t0 + (up1 * t2 - up2 * t1));
+  u[1] = sc * (up1 + ut * t1 + (up2 * t0 - up0 * t2));
+  u[2] = sc * (up2 + ut * t2 + (up0 * t1 - up1 * t0));
+}
+
+// step 2c with the pusher the simulation was created with (warp-uniform branch)
+template <class R>
+__device__ __forceinline__ void push_momentum(int pusher, R kq, R inv_c2, const R* E, const R* B, R* u) {
+  if (pusher) vay<R>(kq, inv_c2, E, B, u);
+  else boris<R>(kq, inv_c2, E, B, u);
 }
 
 // ------------------------------------------------------------------ Esirkepov, per axis set-up

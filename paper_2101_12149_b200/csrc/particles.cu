@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(128) k_particles_global(Grid<R> g, Particles<R
   R w = p.w[t];
   R E[3], B[3];
   gather6<R, ORDER>(g, x0[0], x0[1], x0[2], E, B);
-  boris<R>(p.kq, g.inv_c2, E, B, u);
+  push_momentum<R>(g.pusher, p.kq, g.inv_c2, E, B, u);
   R ig = g.dt / sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * g.inv_c2);
   R x1[3] = {x0[0] + u[0] * ig, x0[1] + u[1] * ig, x0[2] + u[2] * ig};
   deposit_global<R, ORDER>(g, p.jf, w, x0, x1);
@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(128) k_push(Grid<R> g, Particles<R> p, R* __re
   R u[3] = {p.ux[t], p.uy[t], p.uz[t]};
   R E[3], B[3];
   gather6<R, ORDER>(g, x0[0], x0[1], x0[2], E, B);
-  boris<R>(p.kq, g.inv_c2, E, B, u);
+  push_momentum<R>(g.pusher, p.kq, g.inv_c2, E, B, u);
   R ig = g.dt / sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * g.inv_c2);
   xn[t] = x0[0] + u[0] * ig;
   yn[t] = x0[1] + u[1] * ig;

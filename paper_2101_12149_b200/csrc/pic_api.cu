@@ -136,6 +136,8 @@ struct Sim : SimBase {
     g.cJ = (R)(dt_ / kEps0);
     g.inv_c2 = (R)(1.0 / (kC * kC));
     g.dt = (R)dt_;
+    g.pusher = o.pusher;
+    g.gather_mode = o.gather_mode;
     // one allocation for the nine field arrays
     R* base = palloc<R>((size_t)tot * 9);
     if (!base) return fail(PIC_ERR_OOM, "field allocation failed");
@@ -538,6 +540,8 @@ void pic_default_options(pic_options* o) {
   o->sort_interval = 4;
   o->sort_key_mode = 0;
   o->deposit_mode = PIC_DEPOSIT_AUTO;
+  o->pusher = PIC_PUSHER_BORIS;
+  o->gather_mode = PIC_GATHER_UNIFORM;
   o->cuda_stream = nullptr;
 }
 
@@ -554,7 +558,7 @@ int pic_create(const int32_t n_cells[3], const double dx[3], double dt, int shap
   if (shape_order < 1 || shape_order > 3) return bad(PIC_ERR_INVALID_ARG, "shape_order must be 1, 2 or 3");
   if (prec != PIC_F64 && prec != PIC_F32) return bad(PIC_ERR_INVALID_ARG, "unknown precision");
   if (o.sort_interval < 0 || o.sort_key_mode < 0 || o.sort_key_mode > 1 || o.reserved != 0 || o.deposit_mode < 0 ||
-      o.deposit_mode > 4)
+      o.deposit_mode > 4 || o.pusher < 0 || o.pusher > 1 || o.gather_mode < 0 || o.gather_mode > 1)
     return bad(PIC_ERR_INVALID_ARG, "bad option value");
   double s2 = 0;
   for (int d = 0; d < 3; ++d) {

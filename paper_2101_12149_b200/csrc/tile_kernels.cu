@@ -72,11 +72,11 @@ __device__ __forceinline__ R interp_box(const R* __restrict__ F, int base, const
   return acc;
 }
 
-template <class R>
+template <class R, bool GENERIC>
 __device__ __forceinline__ void push_store(const Grid<R>& g, const Particles<R>& p, R* __restrict__ xn,
                                            R* __restrict__ yn, R* __restrict__ zn, int t, const R* x0, R* u,
                                            const R* Ef, const R* Bf) {
-  boris<R>(p.kq, g.inv_c2, Ef, Bf, u);
+  push_momentum<R>(GENERIC ? g.pusher : 0, p.kq, g.inv_c2, Ef, Bf, u);
   R ig = g.dt / sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * g.inv_c2);
   xn[t] = x0[0] + u[0] * ig;
   yn[t] = x0[1] + u[1] * ig;
@@ -84,7 +84,9 @@ __device__ __forceinline__ void push_store(const Grid<R>& g, const Particles<R>&
   p.ux[t] = u[0]; p.uy[t] = u[1]; p.uz[t] = u[2];
 }
 
-template <class R, int ORDER>
+// GENERIC = false: Boris pusher and uniform-order gather, fixed at compile time (the default and the
+// benchmarked path); true: pusher and gather variant read from the Grid (PIC_PUSHER_*, PIC_GATHER_*).
+template <class R, int ORDER, bool GENERIC>
 __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn,
                                                                    R* __restrict__ yn, R* __restrict__ zn,
                                                                    const int32_t* __restrict__ tile_start, TileSpec ts) {
@@ -124,7 +126,9 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
     for (int d = 0; d < 3; ++d) {
       R xi = x0[d] * g.inv_dx[d];
       ln[d] = shape<R, ORDER>(xi, wn[d]) - (d == 0 ? o0 : (d == 1 ? o1 : o2));
-      ls[d] = shape<R, ORDER>(xi - R(0.5), ws[d]) - (d == 0 ? o0 : (d == 1 ? o1 : o2));
+      ls[d] = ((GENERIC && g.gather_mode) ? shape_lowered<R, ORDER>(xi - R(0.5), ws[d])
+                                         : shape<R, ORDER>(xi - R(0.5), ws[d])) -
+              (d == 0 ? o0 : (d == 1 ? o1 : o2));
       inbox &= (ln[d] >= 0) & (ln[d] <= E - ORDER - 1) & (ls[d] >= 0) & (ls[d] <= E - ORDER - 1);
     }
     if (!inbox) {
@@ -133,8 +137,8 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
       const int slot = atomicAdd(&s_ndrift, 1);
       if (slot < PB::MAXD) { s_drift[slot] = t; continue; }
       R Ef[3], Bf[3];
-      gather6<R, ORDER>(g, x0[0], x0[1], x0[2], Ef, Bf);
-      push_store<R>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
+      gather6<R, ORDER, GENERIC>(g, x0[0], x0[1], x0[2], Ef, Bf);
+      push_store<R, GENERIC>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
       continue;
     }
     R Ef[3], Bf[3];
@@ -145,7 +149,7 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
     Bf[0] = interp_box<R, ORDER>(box + 3 * VOL, SX * ln[0] + ls[1] + E * ls[2], wn[0], ws[1], ws[2]);
     Bf[1] = interp_box<R, ORDER>(box + 4 * VOL, SX * ls[0] + ln[1] + E * ls[2], ws[0], wn[1], ws[2]);
     Bf[2] = interp_box<R, ORDER>(box + 5 * VOL, SX * ls[0] + ls[1] + E * ln[2], ws[0], ws[1], wn[2]);
-    push_store<R>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
+    push_store<R, GENERIC>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
   }
   __syncthreads();
   const int nd = min(s_ndrift, PB::MAXD);
@@ -154,8 +158,8 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
     R x0[3] = {p.x[t], p.y[t], p.z[t]};
     R u[3] = {p.ux[t], p.uy[t], p.uz[t]};
     R Ef[3], Bf[3];
-    gather6<R, ORDER>(g, x0[0], x0[1], x0[2], Ef, Bf);
-    push_store<R>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
+    gather6<R, ORDER, GENERIC>(g, x0[0], x0[1], x0[2], Ef, Bf);
+    push_store<R, GENERIC>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
   }
 }
 
@@ -706,14 +710,20 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, bool m
   const size_t vec_smem = (size_t)kW * 32 * TWin<ORDER>::REC * sizeof(R);
   const size_t mma_smem = (size_t)mw * 33 * MWin<ORDER>::REC * sizeof(R);
   if (!attr_set) {
-    cudaFuncSetAttribute(k_push_tile<R, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
+    cudaFuncSetAttribute(k_push_tile<R, ORDER, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
+    cudaFuncSetAttribute(k_push_tile<R, ORDER, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
     cudaFuncSetAttribute(kvec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vec_smem);
     cudaFuncSetAttribute(kmma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mma_smem);
     attr_set = true;
   }
   {
     ScopedPhase ph(c, kPhasePush);
-    k_push_tile<R, ORDER><<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles);
+    if (g.pusher == 0 && g.gather_mode == 0)
+      k_push_tile<R, ORDER, false><<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start,
+                                                                                     a.tiles);
+    else
+      k_push_tile<R, ORDER, true><<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start,
+                                                                                    a.tiles);
   }
   {
     ScopedPhase ph(c, kPhaseDeposit);

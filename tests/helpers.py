@@ -5,7 +5,8 @@ import numpy as np
 import workloads as W
 
 
-def make_pair(cfg, fields="config", shuffle=True, gpu_kwargs=None, with_oracle=True, rng_fields_seed=77):
+def make_pair(cfg, fields="config", shuffle=True, gpu_kwargs=None, with_oracle=True, rng_fields_seed=77,
+              method=None):
     """(oracle or None, gpu Sim, species arrays) for a workloads.Config."""
     import oracle
     import paper_2101_12149_b200 as pic
@@ -13,6 +14,7 @@ def make_pair(cfg, fields="config", shuffle=True, gpu_kwargs=None, with_oracle=T
     if fields == "random":
         E, B = W.random_fields(cfg, np.random.default_rng(rng_fields_seed))
     kw = dict(periodic=cfg.periodic, tile=cfg.tile, sort_interval=cfg.sort_interval)
+    kw.update(method or {})          # pusher= / gather_mode=, same values on both sides
     o = None
     if with_oracle:
         o = oracle.Oracle(cfg.n_cells, cfg.dx, cfg.dt, cfg.order, dtype=cfg.np_dtype, **kw)

@@ -116,6 +116,45 @@ def test_tile_path_steps_between_sorts(order, tile, mode):
     assert d["deactivated"] == 0
 
 
+# ------------------------------------------------------------------ SURVEY.md 8(f) NEXT-2 / NEXT-4
+@pytest.mark.parametrize("order", [1, 2, 3])
+@pytest.mark.parametrize("method", [dict(pusher=1), dict(gather_mode=1), dict(pusher=1, gather_mode=1)])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_vay_pusher_and_galerkin_gather_fp64(order, method, mode):
+    """Vay pusher / Galerkin gather on the tile path (mode 0, steps after the first sort,
+    drifted particles included) and on the fused per-particle kernel (mode 1); relativistic momenta so
+    that the two pushers differ at first order."""
+    cfg = small("C2", (24, 16, 16), order=order, dx=(1.0e-6, 0.8e-6, 0.6e-6))
+    cfg.species[0].sigma = 0.6
+    o, g, _ = make_pair(cfg, fields="random", gpu_kwargs=dict(deposit_mode=mode), method=method)
+    o.step(1); g.step(1)
+    compare_state(o, g, TOL64)
+    o.step(2); g.step(2)
+    compare_state(o, g, 20 * TOL64)
+
+
+def test_vay_and_galerkin_change_the_result():
+    """The options are not silently ignored: each changes u after one step by far more than roundoff
+    (1e-16 of max|u|; the random test fields are weak, so the change itself is small)."""
+    cfg = small("C2", (16, 16, 16), order=3)
+    cfg.species[0].sigma = 0.6
+    base = make_pair(cfg, fields="random", with_oracle=False)[1]
+    base.step(1)
+    ub = base.get_particles(0)["ux"]
+    for method in (dict(pusher=1), dict(gather_mode=1)):
+        g = make_pair(cfg, fields="random", with_oracle=False, method=method)[1]
+        g.step(1)
+        assert np.max(np.abs(g.get_particles(0)["ux"] - ub)) > 1e-11 * np.max(np.abs(ub))
+
+
+def test_vay_and_galerkin_fp32():
+    cfg = small("C3", (16, 16, 16), order=3)
+    cfg.species[0].sigma = 0.3
+    o, g, _ = make_pair(cfg, fields="random", method=dict(pusher=1, gather_mode=1))
+    o.step(2); g.step(2)
+    compare_state(o, g, 4 * TOL32)
+
+
 def test_tile_path_fp32_steps_between_sorts():
     cfg = small("C3", (16, 24, 16), order=3)
     cfg.species[0].sigma = 0.4
