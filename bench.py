@@ -266,6 +266,18 @@ def run_ours(args):
     dist = init_dist("nccl")
     dev = torch.device("cuda", local)
     cfg = W.CONFIGS[args.config]
+    # Fig. 1-style sweeps: same recipe, other sort cadence /
+    # bin size / temperature. The default run leaves the configuration untouched.
+    over = {}
+    if args.sort_interval is not None:
+        over["sort_interval"] = args.sort_interval
+    if args.tile is not None:
+        over["tile"] = tuple(int(v) for v in args.tile.split(","))
+    if over or args.sigma is not None:
+        cfg = W.scaled(cfg, cfg.n_cells, name=cfg.name, **over)
+        if args.sigma is not None:
+            for sp in cfg.species:
+                sp.sigma = args.sigma
     if rank != 0:
         cfg = W.scaled(cfg, cfg.n_cells, name=cfg.name, seed=cfg.seed + 7919 * rank)   # replicas draw their own inputs
     species, E0, B0 = W.generate(cfg)
@@ -275,7 +287,7 @@ def run_ours(args):
     n_cell = cfg.n_cells[0] * cfg.n_cells[1] * cfg.n_cells[2]
     stream = torch.cuda.current_stream()
     kw = dict(dtype=np_dt, periodic=cfg.periodic, tile=cfg.tile, sort_interval=cfg.sort_interval,
-              deposit_mode=args.deposit_mode, stream=stream.cuda_stream)
+              deposit_mode=args.deposit_mode, sort_key_mode=args.sort_key_mode, stream=stream.cuda_stream)
 
     # ---------------- leg 1: state resident in HBM
     sim = pic.Sim(cfg.n_cells, cfg.dx, cfg.dt, cfg.order, **kw)
@@ -449,6 +461,10 @@ def main(argv=None):
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C2", choices=sorted(W.CONFIGS))
     ap.add_argument("--deposit-mode", type=int, default=0, help="PIC_DEPOSIT_* (0 auto, 1 global, 2 cooperative, 3 tile, 4 tile + fp64 tensor pipe)")
+    ap.add_argument("--sort-interval", type=int, default=None, help="sweeps: sort every N steps (0 = only never)")
+    ap.add_argument("--tile", default=None, help="sweeps: cells per sort bin, e.g. 4,4,4")
+    ap.add_argument("--sort-key-mode", type=int, default=0, help="sweeps: 0 cell key inside the tile, 1 tile only")
+    ap.add_argument("--sigma", type=float, default=None, help="sweeps: thermal momentum spread u/c of every species")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs: device-resident leg only")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs: do not time the oracle")
     ap.add_argument("--traffic", type=float, default=None,

@@ -313,7 +313,9 @@ struct Sim : SimBase {
 
   // AUTO: the warp-cooperative deposition needs the cell-sorted order to pay off
   int pick_mode(const Species<R>& sp) const {
-    const bool tiles_ok = sp.sorted_once && tile.T[0] <= 8 && tile.T[1] <= 8 && tile.T[2] <= 8;
+    // the tile kernels want bins of at most 8 cells per axis and enough cells to pay for a CTA
+    const bool tiles_ok = sp.sorted_once && tile.T[0] <= 8 && tile.T[1] <= 8 && tile.T[2] <= 8 &&
+                          (deposit_mode != PIC_DEPOSIT_AUTO || tile.T[0] * tile.T[1] * tile.T[2] >= 64);
     const bool want_tile = deposit_mode == PIC_DEPOSIT_TILE || deposit_mode == PIC_DEPOSIT_TILE_MMA;
     if (want_tile && !tiles_ok) return sp.sorted_once ? kDepositCoop : kDepositGlobal;
     if (deposit_mode != PIC_DEPOSIT_AUTO) return deposit_mode;
