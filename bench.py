@@ -418,17 +418,19 @@ def run_ours(args):
         roof = {"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_frac}
     # dram bytes per launch of that kernel from the committed ncu --set full summary (same workload)
     traffic, traffic_src = args.traffic, ("--traffic" if args.traffic is not None else None)
+    smem_frac = None            # shared-memory wavefronts / peak from the same ncu capture (the push's real bound)
     if traffic is None:
         try:
             tj = json.load(open(os.path.join(ROOT, "profiles", "traffic_%s.json" % cfg.name)))
             key = [k for k in tj["dram_bytes_per_launch"] if k in name]
             if key and args.deposit_mode == 0:
                 traffic, traffic_src = float(tj["dram_bytes_per_launch"][key[0]]), tj["source"]
+                smem_frac = tj.get("shared_wavefront_frac_of_peak", {}).get(key[0])
         except Exception:
             pass
     roof.update({
         "kernel": name, "ms_per_launch": per_launch[dom], "launches_timed": phases[dom][1],
-        "traffic": traffic, "traffic_source": traffic_src, "hbm_gbs": hbm_ach, "hbm_frac": hbm_frac, "alu_tflops": alu_ach,
+        "traffic": traffic, "traffic_source": traffic_src, "shared_wavefront_frac_ncu": smem_frac, "hbm_gbs": hbm_ach, "hbm_frac": hbm_frac, "alu_tflops": alu_ach,
         "alu_frac": alu_frac, "bytes_per_particle": bpp, "flops_per_particle": fpp,
         "peak_source": hbm_src + "; alu = 148 SM x %d FMA/clk x 2 x %.0f MHz" % (per_clk, sm_max),
         "phase_ms_per_step": {k: v[0] / args.steps for k, v in phases.items()},
