@@ -355,3 +355,82 @@ def test_pool_makes_no_allocations_in_steady_state():
     d1 = g.diagnostics()
     assert d1["pool_chunks"] == d0["pool_chunks"] and d1["pool_bytes"] == d0["pool_bytes"]
     assert d1["launches"] > d0["launches"]
+
+
+# ------------------------------------------------------------------ full size, launch configuration of bench.py
+@pytest.mark.parametrize("name,tol", [("C2", TOL64), ("C3", TOL32)])
+def test_full_size_sampled_parity_and_invariants(name, tol):
+    """BASELINE.json configs 2 and 3 at full size (128^3 cells, 16.8 M particles; order 3 fp64 / order 1
+    fp32); C2 is the workload and launch configuration bench.py times. The oracle cannot run it whole in test time, so:
+    (1) sort: cell indices bit-exact against the rule evaluated in numpy, keys non-decreasing, ties in
+        ascending old index, perm a permutation (properties that define the unique stable sort);
+    (2) a sampled sub-box: every particle near it is pushed and deposited by the oracle one by one from
+        the GPU's state after step 1, and x, u of those particles and J on the inner nodes of the box must
+        match the GPU's step 2 to the one-step tolerance;
+    (3) invariants at any size: charge exact, Gauss residual constant."""
+    import oracle
+    cfg = W.CONFIGS[name]
+    _, g, species = make_pair(cfg, with_oracle=False)
+    x_in = [species[0][1][k] for k in "xyz"]                            # as inserted (id = index)
+    n = cfg.n_cells
+    d0 = g.diagnostics()
+    g.step(1)
+    # (1) the sort of step 0
+    cell, perm = g.get_sort_state(0)
+    npart = cfg.n_particles
+    assert np.array_equal(np.sort(perm), np.arange(npart, dtype=perm.dtype))
+    want = np.zeros(npart, dtype=np.int64)
+    for a in (2, 1, 0):       # S-rule: one rounded multiply, floor, clamp; cell = cx + Nx (cy + Ny cz)
+        ca = np.clip(np.floor(x_in[a][perm] * cfg.np_dtype(1.0 / cfg.dx[a])).astype(np.int64), 0, n[a] - 1)
+        want = want * n[a] + ca
+    assert np.array_equal(cell.astype(np.int64), want)
+    del want, x_in
+    T = cfg.tile
+    ci, cj, ck = cell % n[0], (cell // n[0]) % n[1], cell // (n[0] * n[1])
+    nt = (n[0] // T[0], n[1] // T[1], n[2] // T[2])
+    key = ((ci // T[0]) + nt[0] * ((cj // T[1]) + nt[1] * (ck // T[2]))).astype(np.int64) * (T[0] * T[1] * T[2]) + \
+        (ci % T[0]) + T[0] * ((cj % T[1]) + T[1] * (ck % T[2]))
+    dk = np.diff(key)
+    assert np.all(dk >= 0)
+    assert np.all(np.diff(perm.astype(np.int64))[dk == 0] > 0)          # stable: ties keep ascending old index
+    del key, dk, ci, cj, ck
+    p1 = g.get_particles(0)
+    E1, B1, _ = g.get_fields()
+    assert np.array_equal(p1["id"], perm.astype(np.int64))              # id = insertion index, carried through the sort
+    # (2) sampled sub-box, oracle one by one
+    lo, hi, margin = 40, 52, 3
+    cc = [np.floor(p1[k].astype(np.float64) / cfg.dx[a]).astype(np.int64) for a, k in enumerate("xyz")]
+    sel = np.ones(npart, dtype=bool)
+    for a in range(3):
+        sel &= (cc[a] >= lo - margin) & (cc[a] < hi + margin)
+    idx = np.nonzero(sel)[0]
+    assert 30000 < len(idx) < 200000
+    o = oracle.Oracle(n, cfg.dx, cfg.dt, cfg.order, dtype=cfg.np_dtype, sort_interval=0)
+    o.set_fields(E1, B1)
+    spec = cfg.species[0]
+    o.add_species(*[p1[k][idx] for k in ("x", "y", "z", "ux", "uy", "uz", "w")], spec.charge, spec.mass)
+    o.particle_step()
+    g.step(1)
+    p2 = g.get_particles(0)
+    assert np.array_equal(p2["id"], p1["id"])                           # no sort at step 1
+    po = o.get_particles(0)
+    assert family_err([p2[k][idx] for k in "xyz"], [po[k] for k in "xyz"]) <= tol
+    assert family_err([p2[k][idx] for k in ("ux", "uy", "uz")], [po[k] for k in ("ux", "uy", "uz")]) <= tol
+    _, _, Jg = g.get_fields()
+    _, _, Jo = o.get_fields()
+    sl = (slice(lo, hi),) * 3
+    scale = max(np.max(np.abs(J)) for J in Jg)
+    assert scale > 0
+    # fp32 at 128 cells per axis: one ulp of a position is eps32 * 128 = 7.6e-6 cell, the displacement of a
+    # step is ~6e-3 cell, so a last-bit difference in x_new (the two sides contract the push differently)
+    # changes that particle's DS = S1 - S0 by ~1e-3 of itself; ~64 contributions per node leave <~ 1e-4 of
+    # max|J| (DESIGN.md "Tolerances"). x and u themselves meet 1e-5; so do the 16-24 cell one-step cases.
+    tol_J = tol if tol == TOL64 else 1e-4
+    for c in range(3):
+        assert np.max(np.abs(Jg[c][sl].astype(np.float64) - Jo[c][sl])) <= tol_J * scale
+    # (3) invariants
+    g.step(6)                                                           # through the re-sort at step 4
+    d = g.diagnostics()
+    assert d["charge"] == pytest.approx(d0["charge"], rel=1e-12)
+    assert abs(d["gauss_max"] - d0["gauss_max"]) < (1e-9 if tol == TOL64 else 1e-3) * d0["rho_max"]
+    assert d["deactivated"] == 0
