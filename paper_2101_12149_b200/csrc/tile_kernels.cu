@@ -477,6 +477,8 @@ __device__ __forceinline__ void dmma_884(double& c0, double& c1, double a, doubl
                : "d"(a), "d"(b));
 }
 
+__device__ __forceinline__ void prefetch_l2(const void* ptr) { asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr)); }
+
 template <int ORDER>
 struct MWin {
   using T = TWin<ORDER>;
@@ -584,6 +586,11 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
     R x1[3] = {0, 0, 0};
     R w = 0;
     int code = -1;
+    if (tp + 32 < we) {   // the next round's particle data on its way to L2 while this round computes
+      prefetch_l2(p.x + tp + 32); prefetch_l2(p.y + tp + 32); prefetch_l2(p.z + tp + 32);
+      prefetch_l2(xn + tp + 32); prefetch_l2(yn + tp + 32); prefetch_l2(zn + tp + 32);
+      prefetch_l2(p.w + tp + 32);
+    }
     if (valid) {
       R x0[3] = {p.x[tp], p.y[tp], p.z[tp]};
       x1[0] = xn[tp]; x1[1] = yn[tp]; x1[2] = zn[tp];
