@@ -284,6 +284,75 @@ __global__ void __launch_bounds__(128) k_deposit_list(Grid<R> g, Particles<R> p,
   }
 }
 
+// The same per-particle deposit, one WARP per listed particle: lanes 0..2 set up one axis each (compact
+// window of ORDER+2 nodes: S0, DS, running sum of DS) in shared memory, then the 32 lanes walk the
+// particle's nodes with x fastest, so that one RED instruction covers runs of 4-5 contiguous elements
+// instead of 32 unrelated ones (L2 reduction throughput is about 2x better for contiguous lanes).
+template <class R, int ORDER>
+__global__ void __launch_bounds__(128) k_deposit_list_warp(Grid<R> g, Particles<R> p, R* __restrict__ xn,
+                                                           R* __restrict__ yn, R* __restrict__ zn,
+                                                           const int32_t* __restrict__ list,
+                                                           const unsigned int* __restrict__ count,
+                                                           unsigned long long* deactivated) {
+  constexpr int NW = ORDER + 2;
+  __shared__ R s_ax[4][3][3][NW];   // [warp][axis][S0 | DS | prefix of DS][slot]
+  __shared__ int s_b[4][3];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned n = *count;
+  const unsigned nwarps = gridDim.x * (blockDim.x >> 5);
+  const R half = R(0.5), third = R(1) / R(3);
+  for (unsigned e = blockIdx.x * (blockDim.x >> 5) + warp; e < n; e += nwarps) {
+    const int t = list[e];
+    const R w = p.w[t];
+    if (lane < 3) {
+      const R* a0 = lane == 0 ? p.x : (lane == 1 ? p.y : p.z);
+      const R* a1 = lane == 0 ? xn : (lane == 1 ? yn : zn);
+      R S0[NW], DS[NW];
+      int b = esirkepov_axis<R, ORDER>(a0[t] * g.inv_dx[lane], a1[t] * g.inv_dx[lane], S0, DS);
+      b = min(max(b, -kGuard), g.N[lane] + kGuard - NW);
+      s_b[warp][lane] = b;
+      R pre = 0;
+#pragma unroll
+      for (int i = 0; i < NW; ++i) {
+        pre += DS[i];
+        s_ax[warp][lane][0][i] = S0[i];
+        s_ax[warp][lane][1][i] = DS[i];
+        s_ax[warp][lane][2][i] = pre;
+      }
+    }
+    __syncwarp();
+    const int base = g.idx(s_b[warp][0], s_b[warp][1], s_b[warp][2]);
+    // component d: prefix along axis d (NW-1 slots), full windows along the other two (a, b)
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const int a = d == 0 ? 1 : 0, b = d == 2 ? 1 : 2;          // the other two axes, a < b
+      const R f = -(w * p.jf[d]);
+      const int n0 = d == 0 ? NW - 1 : NW, n1 = d == 1 ? NW - 1 : NW, n2 = d == 2 ? NW - 1 : NW;
+      for (int q = lane; q < n0 * n1 * n2; q += 32) {
+        const int i = q % n0, j = (q / n0) % n1, k = q / (n0 * n1);
+        const int sl[3] = {i, j, k};
+        const R S0a = s_ax[warp][a][0][sl[a]], DSa = s_ax[warp][a][1][sl[a]];
+        const R S0b = s_ax[warp][b][0][sl[b]], DSb = s_ax[warp][b][1][sl[b]];
+        const R c = S0a * S0b + half * DSa * S0b + half * S0a * DSb + third * DSa * DSb;
+        const R v = f * (s_ax[warp][d][2][sl[d]] * c);
+        if (v != R(0)) red_add(g.J[d] + base + i + g.sy * j + g.sz * k, v);
+      }
+    }
+    if (lane == 0) {
+      R x1[3] = {xn[t], yn[t], zn[t]};
+      bool out = false;
+#pragma unroll
+      for (int dd = 0; dd < 3; ++dd) out |= wrap_axis<R>(x1[dd], g.L[dd], g.periodic[dd]);
+      if (out) {
+        if (w != R(0)) atomicAdd(deactivated, 1ull);
+        p.w[t] = R(0);
+      }
+      xn[t] = x1[0]; yn[t] = x1[1]; zn[t] = x1[2];
+    }
+    __syncwarp();
+  }
+}
+
 template <class R, int ORDER>
 bool launch_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) {
   const Particles<R>& p = a.cur;
@@ -308,8 +377,8 @@ bool launch_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) 
     cudaMemsetAsync(a.stray_count, 0, 2 * sizeof(unsigned int), c.stream);
     launch_tile_kernels<R>(g, a, ORDER, mode == kDepositTileMma, c);
     ScopedPhase ph(c, kPhaseStray);
-    k_deposit_list<R, ORDER><<<148 * 8, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count,
-                                                           a.deactivated);
+    k_deposit_list_warp<R, ORDER><<<148 * 16, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count,
+                                                                 a.deactivated);
     c.launches += 1;
     return true;
   }
