@@ -52,7 +52,7 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_hist(const uint32_t* __r
 // [w*kPerWarp, (w+1)*kPerWarp) of the block's chunk and walks them 32 at a time; the rank of a
 // key among equal digits is (count in earlier blocks) + (count in earlier warps of the block)
 // + (count earlier in this warp's walk) + (lower lanes with the same digit).
-__global__ void __launch_bounds__(kSortThreads) k_radix_scatter(const uint32_t* __restrict__ keys_in,
+__global__ void __launch_bounds__(kSortThreads, 4) k_radix_scatter(const uint32_t* __restrict__ keys_in,
                                                                 const uint32_t* __restrict__ vals_in,
                                                                 uint32_t* __restrict__ keys_out,
                                                                 uint32_t* __restrict__ vals_out, int64_t n, int shift,
@@ -63,14 +63,18 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(const uint32_t* 
   __syncthreads();
   const int64_t wbase = (int64_t)blockIdx.x * kSortChunk + (int64_t)warp * kPerWarp;
   constexpr int kRounds = kPerWarp / 32;
-  uint32_t key[kRounds], val[kRounds], rank[kRounds];
+  uint32_t key[kRounds], rank[kRounds];   // values are re-read at the end: registers buy occupancy here
   const uint32_t lt = (1u << lane) - 1u;
+  // all loads first (independent, in flight together), then the serial ranking walk
+#pragma unroll
+  for (int r = 0; r < kRounds; ++r) {
+    int64_t p = wbase + r * 32 + lane;
+    key[r] = p < n ? keys_in[p] : 0u;
+  }
 #pragma unroll
   for (int r = 0; r < kRounds; ++r) {
     int64_t p = wbase + r * 32 + lane;
     bool ok = p < n;
-    key[r] = ok ? keys_in[p] : 0u;
-    val[r] = ok ? vals_in[p] : 0u;
     uint32_t d = ok ? ((key[r] >> shift) & 255u) : (256u + lane);   // invalid lanes match nobody
     uint32_t m = __match_any_sync(0xffffffffu, d);
     int leader = __ffs(m) - 1;
@@ -101,7 +105,7 @@ __global__ void __launch_bounds__(kSortThreads) k_radix_scatter(const uint32_t* 
     if (p < n) {
       uint32_t pos = cnt[warp][(key[r] >> shift) & 255u] + rank[r];
       keys_out[pos] = key[r];
-      vals_out[pos] = val[r];
+      vals_out[pos] = vals_in[p];
     }
   }
 }
