@@ -26,6 +26,8 @@ namespace {
 
 constexpr int kTileMax = 8;   // largest tile edge (cells) these kernels are laid out for
 
+__device__ __forceinline__ void prefetch_l2(const void* ptr) { asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr)); }
+
 __device__ __forceinline__ void tile_coords(const TileSpec& ts, int tile, int* tb) {
   int tx = tile % ts.nt[0];
   int r = tile / ts.nt[0];
@@ -119,6 +121,11 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
   for (int t = s + threadIdx.x; t < e; t += blockDim.x) {
     R x0[3] = {p.x[t], p.y[t], p.z[t]};
     R u[3] = {p.ux[t], p.uy[t], p.uz[t]};
+    if (t + (int)blockDim.x < e) {   // the next particle of this thread on its way to L2
+      const int tn = t + blockDim.x;
+      prefetch_l2(p.x + tn); prefetch_l2(p.y + tn); prefetch_l2(p.z + tn);
+      prefetch_l2(p.ux + tn); prefetch_l2(p.uy + tn); prefetch_l2(p.uz + tn);
+    }
     R wn[3][ORDER + 1], ws[3][ORDER + 1];
     int ln[3], ls[3];
     bool inbox = true;
@@ -476,8 +483,6 @@ __device__ __forceinline__ void dmma_884(double& c0, double& c1, double a, doubl
                : "+d"(c0), "+d"(c1)
                : "d"(a), "d"(b));
 }
-
-__device__ __forceinline__ void prefetch_l2(const void* ptr) { asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr)); }
 
 template <int ORDER>
 struct MWin {
