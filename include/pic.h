@@ -186,9 +186,9 @@ PIC_API int pic_get_rho(pic_sim* sim, double* rho, pic_mem where);
  * until pic_enable_phase_timing(sim, 1). pic_get_phase_times synchronises. */
 enum {
   PIC_PHASE_SORT = 0,    /* keys, radix passes, permutation of all attributes */
-  PIC_PHASE_PUSH = 1,    /* gather + Boris push (+ deposit when PIC_DEPOSIT_GLOBAL fuses it) */
-  PIC_PHASE_DEPOSIT = 2, /* warp-cooperative Esirkepov deposition */
-  PIC_PHASE_STRAY = 3,   /* per-particle deposition of the particles the cooperative kernel skipped */
+  PIC_PHASE_PUSH = 1,    /* gather + momentum push (+ deposit when PIC_DEPOSIT_GLOBAL fuses it) */
+  PIC_PHASE_DEPOSIT = 2, /* Esirkepov deposition of the sorted runs (tensor-pipe / lane-group / warp-cooperative kernel) */
+  PIC_PHASE_STRAY = 3,   /* per-particle deposition of the particles that kernel listed instead */
   PIC_PHASE_FIELDS = 4,  /* J zero, J guard sum, Yee B/E/B, guard fill */
   PIC_NPHASE = 5
 };

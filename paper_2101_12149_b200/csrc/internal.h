@@ -87,7 +87,7 @@ enum { kDepositGlobal = 1, kDepositCoop = 2, kDepositTile = 3, kDepositTileMma =
 constexpr int kPushTileThreads = 256;   // k_push_tile: threads per CTA (one CTA per tile)
 constexpr int kDepMmaWarps = 4;         // k_deposit_mma: warps per CTA (one CTA per tile) ...
 constexpr int kDepMmaCtas = 5;          // ... and CTAs per SM the register budget is set for (20 warps per SM)
-constexpr int kDepTileWarps = 8;        // k_deposit_tile / k_deposit_mma: warps per CTA (one CTA per tile, two per SM)
+constexpr int kDepTileWarps = 8;        // k_deposit_tile: warps per CTA (one CTA per tile, two per SM)
 template <class R>
 struct ParticleStep {
   Particles<R> cur;                  // x^n, u^{n-1/2}, w
