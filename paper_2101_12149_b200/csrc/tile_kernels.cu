@@ -28,6 +28,14 @@ constexpr int kTileMax = 8;   // largest tile edge (cells) these kernels are lai
 
 __device__ __forceinline__ void prefetch_l2(const void* ptr) { asm volatile("prefetch.global.L2 [%0];" ::"l"(ptr)); }
 
+// one element global -> shared without passing through registers (cp.async, 4 or 8 bytes)
+template <class R>
+__device__ __forceinline__ void cp_async(R* smem_dst, const R* gmem_src) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+  if constexpr (sizeof(R) == 8) asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(sa), "l"(gmem_src) : "memory");
+  else asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(sa), "l"(gmem_src) : "memory");
+}
+
 __device__ __forceinline__ void tile_coords(const TileSpec& ts, int tile, int* tb) {
   int tx = tile % ts.nt[0];
   int r = tile / ts.nt[0];
@@ -114,9 +122,14 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
     const bool in = (o0 + i < lim0) & (o1 + j < lim1) & (o2 + k < lim2);
     const int gi = g.idx(o0 + i, o1 + j, o2 + k);
     const int li = SX * i + j + E * k;
+    // asynchronous copies (LDGSTS): every element of the box is in flight at once, no register staging
 #pragma unroll
-    for (int c = 0; c < 6; ++c) box[c * VOL + li] = in ? __ldg(g.F[c] + gi) : R(0);
+    for (int c = 0; c < 6; ++c) {
+      if (in) cp_async(box + c * VOL + li, g.F[c] + gi);
+      else box[c * VOL + li] = R(0);
+    }
   }
+  asm volatile("cp.async.wait_all;" ::: "memory");
   __syncthreads();
   for (int t = s + threadIdx.x; t < e; t += blockDim.x) {
     R x0[3] = {p.x[t], p.y[t], p.z[t]};
