@@ -65,8 +65,10 @@ def model(cfg, deposit_split=True):
     boris_f = 110
     nw = n + 2
     dep_f = 3 * (nw * nw * 8 + nw * nw * (nw - 1) * 3) + 6 * (10 if n == 3 else 6 if n == 2 else 2) * 2 + 60
+    # the gather's shared-memory reads in k_push_tile: every stencil value of every component, once per particle
+    push_smem_b = 6 * m ** 3 * P
     return dict(P=P, ppc=ppc, step_bytes=step, push_bytes=push_b, deposit_bytes=dep_b, fused_bytes=fused_b,
-                push_flops=gather_f + boris_f, deposit_flops=dep_f)
+                push_flops=gather_f + boris_f, deposit_flops=dep_f, push_smem_bytes=push_smem_b)
 
 
 # ----------------------------------------------------------------------------- clocks
@@ -435,6 +437,13 @@ def run_ours(args):
         "peak_source": hbm_src + "; alu = 148 SM x %d FMA/clk x 2 x %.0f MHz" % (per_clk, sm_max),
         "phase_ms_per_step": {k: v[0] / args.steps for k, v in phases.items()},
     })
+    if dom == "push" and not fused:
+        # the roof that actually binds k_push_tile: shared-memory bandwidth,
+        # 148 SMs x 128 B/clk x SM clock; achieved = algorithmic stencil bytes / launch time
+        smem_peak = N_SM * 128 * sm_max * 1e6 / 1e12
+        smem_ach = m["push_smem_bytes"] * units / dur / 1e12 if dur > 0 else 0.0
+        roof["smem"] = {"achieved": smem_ach, "peak": smem_peak, "unit": "TB/s", "frac": smem_ach / smem_peak,
+                        "bytes_per_particle": m["push_smem_bytes"]}
     step_gbs = m["step_bytes"] * n_part * args.steps / (ms * 1e-3) / 1e9
 
     cpu = None
