@@ -57,6 +57,9 @@ def lib():
         L.orc_particle_step.argtypes = [vp]
         L.orc_shape_f64.argtypes = [C.c_int, C.c_double, i32p, dp]
         L.orc_shape_f32.argtypes = [C.c_int, C.c_float, i32p, C.POINTER(C.c_float)]
+        L.orc_create_ex.restype = vp
+        L.orc_create_ex.argtypes = L.orc_create.argtypes + [C.c_int]
+        L.orc_ckc_coefficients.argtypes = [vp, dp]
         L.orc_set_method.argtypes = [vp, C.c_int, C.c_int]
         L.orc_set_method.restype = C.c_int
         L.orc_vay_f64.argtypes = [C.c_double, dp, dp, dp]
@@ -114,6 +117,7 @@ def vay(kq: float, E, B, u, dtype=np.float64):
 
 
 PUSHER_BORIS, PUSHER_VAY = 0, 1
+SOLVER_YEE, SOLVER_CKC = 0, 1
 GATHER_UNIFORM, GATHER_GALERKIN = 0, 1
 
 
@@ -121,7 +125,8 @@ class Oracle:
     """One oracle simulation. Arrays in and out are numpy, x-fastest fields of shape (nz, ny, nx)."""
 
     def __init__(self, n_cells, dx, dt, order, dtype=np.float64, periodic=(1, 1, 1), tile=(8, 8, 8),
-                 sort_interval=4, sort_key_mode=0, pusher=PUSHER_BORIS, gather_mode=GATHER_UNIFORM):
+                 sort_interval=4, sort_key_mode=0, pusher=PUSHER_BORIS, gather_mode=GATHER_UNIFORM,
+                 solver=SOLVER_YEE):
         self.dtype = np.dtype(dtype)
         self.n_cells = tuple(int(v) for v in n_cells)
         self.dx = tuple(float(v) for v in dx)
@@ -129,14 +134,21 @@ class Oracle:
         self.order = int(order)
         tile = tuple(min(int(t), n) for t, n in zip(tile, self.n_cells))
         dxa = (C.c_double * 3)(*self.dx)
-        self._h = lib().orc_create(_i32(self.n_cells), dxa, self.dt, self.order,
+        self._h = lib().orc_create_ex(_i32(self.n_cells), dxa, self.dt, self.order,
                                    0 if self.dtype == np.float64 else 1, _i32(periodic), _i32(tile),
-                                   int(sort_interval), int(sort_key_mode))
+                                      int(sort_interval), int(sort_key_mode), int(solver))
         if not self._h:
             raise ValueError("orc_create rejected the arguments (order, tile, dx or CFL)")
         self._fshape = (self.n_cells[2], self.n_cells[1], self.n_cells[0])
         if lib().orc_set_method(self._h, int(pusher), int(gather_mode)) != 0:
             raise ValueError("unknown pusher / gather_mode")
+
+    def ckc_coefficients(self):
+        """(alpha[3], beta[3][3], gamma[3]) of the CKC solver for this grid."""
+        out = (C.c_double * 15)()
+        lib().orc_ckc_coefficients(self._h, out)
+        v = np.array(out[:])
+        return v[:3], v[3:12].reshape(3, 3), v[12:]
 
     def close(self):
         if self._h:

@@ -97,6 +97,8 @@ struct Sim {
   int tile[3];
   int sort_interval, key_mode;
   int pusher = 0;        // 0 Boris (reading Q2), 1 Vay (ref [21])
+  int solver = 0;        // 0 Yee (ref [28]), 1 CKC (Cole-Karkkainen-Cowan, ref [12])
+  R ck_a[3], ck_b[3][3], ck_g[3];   // CKC: alpha_a, beta_ab (b != a), gamma_a, in working precision
   int gather_mode = 0;   // 0 uniform order (reading Q1), 1 Galerkin / energy-conserving (NEXT-2)
   // coefficient block (C-list): computed in double, rounded once to R
   R inv_dx[3], L[3], cB[3], cE[3], cJ, inv_c2, dtr;
@@ -329,6 +331,50 @@ void push_B_half(Sim<R>& s) {
   s.F[3].swap(nBx); s.F[4].swap(nBy); s.F[5].swap(nBz);
 }
 
+// CKC solver (PAPER.md:255 lists it among WarpX's solvers; ref [12] Cowan et al., PRST-AB 16, 041303):
+// the E update is Yee's; in the B update every difference of E along an axis a is replaced by the
+// smoothed difference
+//   D_a F = alpha_a dF(0,0) + beta_ab [dF(+b) + dF(-b)] + beta_ac [dF(+c) + dF(-c)]
+//         + gamma_a [dF(+b,+c) + dF(+b,-c) + dF(-b,+c) + dF(-b,-c)],   dF(s) = F[+1 along a, s] - F[s],
+// b, c the two transverse axes. Coefficients (delta = min dx, r_a = (delta/dx_a)^2, S = r_y r_z + r_z r_x + r_x r_y):
+//   beta = (1 - r_x r_y r_z / S) / 8,  beta_ab = r_b beta,  gamma_a = r_b r_c (1/16 - r_b r_c / (8 S)),
+//   alpha_a = 1 - 2 beta_ab - 2 beta_ac - 4 gamma_a   (cubic cells: 7/12, 1/12, 1/48).
+// They remove the dispersion along the axes at c dt = delta, where the scheme is still stable (pin T15).
+template <class R>
+R ckc_diff(const Sim<R>& s, const std::vector<R>& F, int a, int i, int j, int k) {
+  const int b = (a + 1) % 3, c = (a + 2) % 3;
+  auto dF = [&](int sb, int sc) {
+    int p[3] = {i, j, k};
+    p[b] += sb; p[c] += sc;
+    int q[3] = {p[0], p[1], p[2]};
+    q[a] += 1;
+    return s.rd(F, q[0], q[1], q[2]) - s.rd(F, p[0], p[1], p[2]);
+  };
+  return s.ck_a[a] * dF(0, 0) + s.ck_b[a][b] * (dF(1, 0) + dF(-1, 0)) + s.ck_b[a][c] * (dF(0, 1) + dF(0, -1)) +
+         s.ck_g[a] * (dF(1, 1) + dF(1, -1) + dF(-1, 1) + dF(-1, -1));
+}
+
+template <class R>
+void push_B_half_ckc(Sim<R>& s) {
+  auto &Ex = s.F[0], &Ey = s.F[1], &Ez = s.F[2];
+  std::vector<R> nBx(s.F[3]), nBy(s.F[4]), nBz(s.F[5]);
+  for (int k = 0; k < s.N[2]; ++k)
+    for (int j = 0; j < s.N[1]; ++j)
+      for (int i = 0; i < s.N[0]; ++i) {
+        size_t t = (size_t)s.lin(i, j, k);
+        nBx[t] -= s.cB[1] * ckc_diff<R>(s, Ez, 1, i, j, k) - s.cB[2] * ckc_diff<R>(s, Ey, 2, i, j, k);
+        nBy[t] -= s.cB[2] * ckc_diff<R>(s, Ex, 2, i, j, k) - s.cB[0] * ckc_diff<R>(s, Ez, 0, i, j, k);
+        nBz[t] -= s.cB[0] * ckc_diff<R>(s, Ey, 0, i, j, k) - s.cB[1] * ckc_diff<R>(s, Ex, 1, i, j, k);
+      }
+  s.F[3].swap(nBx); s.F[4].swap(nBy); s.F[5].swap(nBz);
+}
+
+template <class R>
+void push_B(Sim<R>& s) {
+  if (s.solver == 1) push_B_half_ckc<R>(s);
+  else push_B_half<R>(s);
+}
+
 template <class R>
 void push_E(Sim<R>& s) {
   auto &Bx = s.F[3], &By = s.F[4], &Bz = s.F[5];
@@ -388,9 +434,9 @@ void step(Sim<R>& s) {
   particles_step<R>(s);                                             // 2
   for (int c = 0; c < 3; ++c)
     for (size_t t = 0; t < s.ncell(); ++t) s.J[c][t] = (R)s.Jd[c][t];
-  push_B_half<R>(s);                                                // 3
+  push_B<R>(s);                                                     // 3
   push_E<R>(s);                                                     // 4
-  push_B_half<R>(s);                                                // 5
+  push_B<R>(s);                                                     // 5
   s.step_count++;
 }
 
@@ -480,6 +526,21 @@ Sim<R>* make_sim(const int32_t* N, const double* dx, double dt, int order, const
     s->cB[d] = (R)(dt / (2.0 * dx[d]));
     s->cE[d] = (R)(kC * kC * dt / dx[d]);
   }
+  {
+    const double delta = std::min(dx[0], std::min(dx[1], dx[2]));
+    double r[3];
+    for (int d = 0; d < 3; ++d) r[d] = (delta / dx[d]) * (delta / dx[d]);
+    const double S = r[1] * r[2] + r[2] * r[0] + r[0] * r[1];
+    const double beta = 0.125 * (1.0 - r[0] * r[1] * r[2] / S);
+    for (int a = 0; a < 3; ++a) {
+      const int b = (a + 1) % 3, c = (a + 2) % 3;
+      const double bab = r[b] * beta, bac = r[c] * beta;
+      const double ga = r[b] * r[c] * (0.0625 - 0.125 * r[b] * r[c] / S);
+      s->ck_b[a][a] = R(0); s->ck_b[a][b] = (R)bab; s->ck_b[a][c] = (R)bac;
+      s->ck_g[a] = (R)ga;
+      s->ck_a[a] = (R)(1.0 - 2.0 * bab - 2.0 * bac - 4.0 * ga);
+    }
+  }
   s->dt = dt; s->order = order; s->sort_interval = sort_interval; s->key_mode = key_mode;
   s->cJ = (R)(dt / kEps0);
   s->inv_c2 = (R)(1.0 / (kC * kC));
@@ -515,19 +576,38 @@ int add_species(Sim<R>& s, int64_t n, const void* const* arr, double q, double m
 extern "C" {
 
 // --- whole-simulation interface (mirrors the product's calls; reading SURVEY.md §8(b))
-void* orc_create(const int32_t* n_cells, const double* dx, double dt, int order, int prec,
-                 const int32_t* periodic, const int32_t* tile, int sort_interval, int key_mode) {
+// solver: 0 Yee (stable for c dt sqrt(sum 1/dx^2) <= 1), 1 CKC (stable for c dt <= min dx)
+void* orc_create_ex(const int32_t* n_cells, const double* dx, double dt, int order, int prec,
+                    const int32_t* periodic, const int32_t* tile, int sort_interval, int key_mode, int solver) {
   if (order < 1 || order > 3) return nullptr;
   for (int d = 0; d < 3; ++d)
     if (n_cells[d] < 1 || tile[d] < 1 || n_cells[d] % tile[d] != 0 || !(dx[d] > 0)) return nullptr;
   double s2 = 0;
   for (int d = 0; d < 3; ++d) s2 += 1.0 / (dx[d] * dx[d]);
-  if (!(dt > 0) || dt * kC * std::sqrt(s2) > 1.0) return nullptr;      // CFL
+  if (solver < 0 || solver > 1) return nullptr;
+  const double dmin = std::min(dx[0], std::min(dx[1], dx[2]));
+  if (!(dt > 0) || (solver == 0 ? dt * kC * std::sqrt(s2) > 1.0 : dt * kC > dmin * (1.0 + 1e-12))) return nullptr;   // CFL
   auto* h = new Handle();
   h->prec = prec;
   if (prec == 0) h->d = make_sim<double>(n_cells, dx, dt, order, periodic, tile, sort_interval, key_mode);
   else h->f = make_sim<float>(n_cells, dx, dt, order, periodic, tile, sort_interval, key_mode);
+  if (prec == 0) h->d->solver = solver; else h->f->solver = solver;
   return h;
+}
+
+void* orc_create(const int32_t* n_cells, const double* dx, double dt, int order, int prec,
+                 const int32_t* periodic, const int32_t* tile, int sort_interval, int key_mode) {
+  return orc_create_ex(n_cells, dx, dt, order, prec, periodic, tile, sort_interval, key_mode, 0);
+}
+
+// CKC coefficients as the oracle uses them (f64): out[0..2] alpha_a, out[3..11] beta_ab row-major, out[12..14] gamma_a
+void orc_ckc_coefficients(void* hv, double* out) {
+  auto* h = (Handle*)hv;
+  for (int a = 0; a < 3; ++a) {
+    out[a] = h->prec == 0 ? (double)h->d->ck_a[a] : (double)h->f->ck_a[a];
+    out[12 + a] = h->prec == 0 ? (double)h->d->ck_g[a] : (double)h->f->ck_g[a];
+    for (int b = 0; b < 3; ++b) out[3 + 3 * a + b] = h->prec == 0 ? (double)h->d->ck_b[a][b] : (double)h->f->ck_b[a][b];
+  }
 }
 
 void orc_destroy(void* hv) {
@@ -637,8 +717,8 @@ void orc_sort_now(void* hv) {
 void orc_field_step(void* hv, int n) {
   auto* h = (Handle*)hv;
   for (int i = 0; i < n; ++i) {
-    if (h->prec == 0) { push_B_half(*h->d); push_E(*h->d); push_B_half(*h->d); }
-    else { push_B_half(*h->f); push_E(*h->f); push_B_half(*h->f); }
+    if (h->prec == 0) { push_B(*h->d); push_E(*h->d); push_B(*h->d); }
+    else { push_B(*h->f); push_E(*h->f); push_B(*h->f); }
   }
 }
 // zero J, run step 2 for every particle, round J; no sort, no field update

@@ -671,3 +671,113 @@ def test_T14_galerkin_gather_is_the_small_move_limit_of_the_esirkepov_deposit(or
         assert abs(work - (-Q_E) * w[0] * delta * eg) < 1e-6 * scale
         worst_uniform = max(worst_uniform, abs(work - (-Q_E) * w[0] * delta * eu) / scale)
     assert worst_uniform > 1e-3          # the uniform-order gather does NOT satisfy it: the pin discriminates
+
+
+# --------------------------------------------------------------------------- T15 CKC solver (NEXT-4)
+def _ckc_symbol(k, dx, alpha, beta, gamma):
+    """S_a(k) = alpha_a + 2 beta_ab cos(k_b dx_b) + 2 beta_ac cos(k_c dx_c) + 4 gamma_a cos cos: the Fourier
+    symbol of the transverse smoothing of the difference along a."""
+    S = []
+    for a in range(3):
+        b, cc = (a + 1) % 3, (a + 2) % 3
+        cb, cz = math.cos(k[b] * dx[b]), math.cos(k[cc] * dx[cc])
+        S.append(alpha[a] + 2 * beta[a][b] * cb + 2 * beta[a][cc] * cz + 4 * gamma[a] * cb * cz)
+    return np.array(S)
+
+
+def test_T15_ckc_coefficients_cubic_values_consistency_and_von_neumann_stability():
+    """Cubic cells: the published 7/12, 1/12, 1/48 (ref [12]). Any cells: the weights of every smoothed
+    difference sum to 1 (second-order consistency), and with c dt = min(dx) — beyond Yee's limit — the
+    amplification stays on the unit circle for every wave vector: 0 <= (c dt)^2 sum_a S_a sin^2(k_a dx_a/2)
+    / dx_a^2 <= 1 (the property the coefficients are built for)."""
+    o = Oracle((8, 8, 8), (1e-6,) * 3, 1e-6 / c, 1, sort_interval=0, solver=oracle.SOLVER_CKC)
+    al, be, ga = o.ckc_coefficients()
+    assert np.allclose(al, 7 / 12, rtol=1e-15) and np.allclose(ga, 1 / 48, rtol=1e-14)
+    assert np.allclose(be[~np.eye(3, dtype=bool)], 1 / 12, rtol=1e-14)
+    for dx in [(1e-6, 1e-6, 1e-6), (1e-6, 0.8e-6, 0.5e-6), (0.1e-6, 0.1e-6, 0.025e-6), (2e-6, 1e-6, 1e-6)]:
+        dmin = min(dx)
+        dt = dmin / c
+        o = Oracle((8, 8, 8), dx, dt, 1, sort_interval=0, solver=oracle.SOLVER_CKC)
+        al, be, ga = o.ckc_coefficients()
+        for a in range(3):
+            b, cc = (a + 1) % 3, (a + 2) % 3
+            assert abs(al[a] + 2 * be[a][b] + 2 * be[a][cc] + 4 * ga[a] - 1) < 1e-15
+        worst = 0.0
+        for kx in np.linspace(0, math.pi, 25):
+            for ky in np.linspace(0, math.pi, 25):
+                for kz in np.linspace(0, math.pi, 25):
+                    k = np.array([kx / dx[0], ky / dx[1], kz / dx[2]])
+                    S = _ckc_symbol(k, dx, al, be, ga)
+                    s2 = (c * dt) ** 2 * sum(S[a] * math.sin(k[a] * dx[a] / 2) ** 2 / dx[a] ** 2 for a in range(3))
+                    assert s2 > -1e-14
+                    worst = max(worst, s2)
+        assert worst <= 1 + 1e-12
+        assert worst > 0.999                    # the limit is reached: c dt = min(dx) is the edge
+        with pytest.raises(ValueError):         # Yee cannot run this time step
+            Oracle((8, 8, 8), dx, dt, 1, sort_interval=0)
+
+
+@pytest.mark.parametrize("frac", [0.7, 1.0])
+def test_T15_ckc_plane_wave_dispersion(frac):
+    """A discrete plane wave with omega from the CKC relation sin^2(omega dt/2) = (c dt)^2 sum_a S_a(k)
+    sin^2(k_a dx_a/2)/dx_a^2, E perpendicular to K, B = K' x E / Omega with K'_a = S_a K_a, is reproduced to
+    roundoff over hundreds of steps on an anisotropic grid, also at c dt = min(dx)."""
+    n, dx = (8, 12, 16), (1.0e-6, 0.8e-6, 0.5e-6)
+    dt = frac * min(dx) / c
+    o = Oracle(n, dx, dt, 1, tile=(1, 1, 1), sort_interval=0, solver=oracle.SOLVER_CKC)
+    al, be, ga = o.ckc_coefficients()
+    mode = (1, 2, 1)
+    k = np.array([2 * math.pi * mode[d] / (n[d] * dx[d]) for d in range(3)])
+    S = _ckc_symbol(k, dx, al, be, ga)
+    K = np.array([2 / dx[d] * math.sin(k[d] * dx[d] / 2) for d in range(3)])
+    Kp = S * K
+    s2 = (c * dt) ** 2 * sum(S[d] * math.sin(k[d] * dx[d] / 2) ** 2 / dx[d] ** 2 for d in range(3))
+    om = 2 / dt * math.asin(math.sqrt(s2))
+    Om = 2 / dt * math.sin(om * dt / 2)
+    E0 = np.cross(K, [0.3, -0.2, 1.0])
+    E0 *= 1e9 / np.linalg.norm(E0)
+    B0 = np.cross(Kp, E0) / Om
+    stag = [(.5, 0, 0), (0, .5, 0), (0, 0, .5), (0, .5, .5), (.5, 0, .5), (.5, .5, 0)]
+
+    def phase(cmp):
+        xs = (np.arange(n[0]) + stag[cmp][0]) * dx[0]
+        ys = (np.arange(n[1]) + stag[cmp][1]) * dx[1]
+        zs = (np.arange(n[2]) + stag[cmp][2]) * dx[2]
+        return k[0] * xs[None, None, :] + k[1] * ys[None, :, None] + k[2] * zs[:, None, None]
+
+    def exact(t):
+        E = [E0[d] * np.cos(phase(d) - om * t) for d in range(3)]
+        B = [B0[d] * math.cos(om * dt / 2) * np.cos(phase(3 + d) - om * t) for d in range(3)]
+        return E, B
+
+    o.set_fields(*exact(0.0))
+    nsteps = 300
+    o.field_step(nsteps)
+    E, B, _ = o.get_fields()
+    Ee, Be = exact(nsteps * dt)
+    for d in range(3):
+        assert np.max(np.abs(E[d] - Ee[d])) < 1e-11 * 1e9
+        assert np.max(np.abs(B[d] - Be[d])) < 1e-11 * np.linalg.norm(B0)
+    assert om * nsteps * dt > 20
+    # the Yee relation (S = 1) is a different wave: the pin discriminates
+    s2y = (c * dt) ** 2 * sum(math.sin(k[d] * dx[d] / 2) ** 2 / dx[d] ** 2 for d in range(3))
+    assert abs(s2y - s2) > 1e-3 * s2
+
+
+def test_T15_ckc_no_dispersion_along_the_axis_at_the_magic_time_step():
+    """Cubic cells, c dt = dx: a wave along an axis has omega = c k exactly (S = 1 for transverse k = 0,
+    sin(omega dt/2) = sin(k dx/2)), for every resolvable k — the reason the scheme exists."""
+    n, dx = (16, 4, 4), (1e-6, 1e-6, 1e-6)
+    dt = dx[0] / c
+    o = Oracle(n, dx, dt, 1, tile=(1, 1, 1), sort_interval=0, solver=oracle.SOLVER_CKC)
+    rng = np.random.default_rng(151)
+    f = rng.normal(size=n[0]) * 1e9                       # any profile: every Fourier mode moves at c
+    Ey = np.broadcast_to(f[None, None, :], (n[2], n[1], n[0])).copy()
+    zf = np.zeros_like(Ey)
+    # forward wave: Bz(i+1/2) at the integer time = average of the two half-step values f(i), f(i+1) / c
+    Bz = np.broadcast_to(((f + np.roll(f, -1)) / (2 * c))[None, None, :], Ey.shape).copy()
+    o.set_fields([zf, Ey, zf], [zf, zf, Bz])
+    o.field_step(5)
+    E, B, _ = o.get_fields()
+    assert np.max(np.abs(E[1][0, 0, :] - np.roll(f, 5))) < 1e-12 * np.max(np.abs(f))
+    assert np.max(np.abs(E[0])) == 0 and np.max(np.abs(E[2])) == 0
