@@ -89,6 +89,13 @@ enum { PIC_PUSHER_BORIS = 0, PIC_PUSHER_VAY = 1 };
  * staggered ("energy-conserving" gather). */
 enum { PIC_GATHER_UNIFORM = 0, PIC_GATHER_GALERKIN = 1 };
 
+/* Field solver of steps 3-5. YEE: the standard Yee curl (ref [28]); time step limit
+ * dt*c*sqrt(sum 1/dx^2) <= 1. CKC: Cole-Karkkainen-Cowan (ref [12]): the E
+ * update is Yee's, every difference of E in the B update is smoothed over the 3x3 transverse
+ * neighbours with the weights alpha, beta, gamma of DESIGN.md section 11; no dispersion along the
+ * axes at c*dt = min(dx), which is also its time step limit (PIC_ERR_CFL beyond it). */
+enum { PIC_SOLVER_YEE = 0, PIC_SOLVER_CKC = 1 };
+
 /* Options; pass NULL to pic_create for the defaults given here. */
 typedef struct {
   int32_t periodic[3];   /* default {1,1,1}; 0 = truncation with zeroed guard cells on that axis:
@@ -103,7 +110,7 @@ typedef struct {
   int32_t deposit_mode;  /* PIC_DEPOSIT_*; default PIC_DEPOSIT_AUTO */
   int32_t pusher;        /* PIC_PUSHER_*; default PIC_PUSHER_BORIS */
   int32_t gather_mode;   /* PIC_GATHER_*; default PIC_GATHER_UNIFORM */
-  int32_t reserved;      /* must be 0 */
+  int32_t solver;        /* PIC_SOLVER_*; default PIC_SOLVER_YEE */
   void*   cuda_stream;   /* cudaStream_t all work is issued on (e.g. torch's current stream);
                             NULL = the legacy default stream */
 } pic_options;

@@ -21,6 +21,8 @@ struct Grid {
   int periodic[3];
   int pusher;        // PIC_PUSHER_*
   int gather_mode;   // PIC_GATHER_*
+  int solver;        // PIC_SOLVER_*
+  R ck_a[3], ck_b[3][3], ck_g[3];   // CKC weights alpha_a, beta_ab, gamma_a
   R inv_dx[3], L[3], cB[3], cE[3], cJ, inv_c2, dt;
   R* F[6];           // Ex Ey Ez Bx By Bz
   R* J[3];

@@ -8,8 +8,21 @@ namespace {
 
 struct Box3 { int lo[3], n[3]; };
 
-// B -= (dt/2) curl E, forward differences, over the box [lo, lo+n)
-template <class R>
+// CKC (ref [12]): the difference of F along axis A at element t, smoothed over the 3x3 transverse
+// neighbours: alpha dF(0,0) + beta_ab [dF(+b) + dF(-b)] + beta_ac [dF(+c) + dF(-c)] + gamma [4 corners]
+template <class R, int A>
+__device__ __forceinline__ R ckc_diff(const Grid<R>& g, const R* __restrict__ F, int t) {
+  constexpr int B = (A + 1) % 3, C = (A + 2) % 3;
+  const int sa = A == 0 ? 1 : (A == 1 ? g.sy : g.sz);
+  const int sb = B == 0 ? 1 : (B == 1 ? g.sy : g.sz);
+  const int sc = C == 0 ? 1 : (C == 1 ? g.sy : g.sz);
+  auto dF = [&](int o) { return F[t + o + sa] - F[t + o]; };
+  return g.ck_a[A] * dF(0) + g.ck_b[A][B] * (dF(sb) + dF(-sb)) + g.ck_b[A][C] * (dF(sc) + dF(-sc)) +
+         g.ck_g[A] * (dF(sb + sc) + dF(sb - sc) + dF(-sb + sc) + dF(-sb - sc));
+}
+
+// B -= (dt/2) curl E, forward differences (Yee) or CKC-smoothed ones, over the box [lo, lo+n)
+template <class R, bool CKC>
 __global__ void __launch_bounds__(256) k_push_B(Grid<R> g, Box3 b) {
   int i = blockIdx.x * blockDim.x + threadIdx.x;
   int j = blockIdx.y * blockDim.y + threadIdx.y;
@@ -19,10 +32,16 @@ __global__ void __launch_bounds__(256) k_push_B(Grid<R> g, Box3 b) {
   const R* __restrict__ Ex = g.F[0];
   const R* __restrict__ Ey = g.F[1];
   const R* __restrict__ Ez = g.F[2];
-  R ex = Ex[t], ey = Ey[t], ez = Ez[t];
-  g.F[3][t] -= g.cB[1] * (Ez[t + g.sy] - ez) - g.cB[2] * (Ey[t + g.sz] - ey);
-  g.F[4][t] -= g.cB[2] * (Ex[t + g.sz] - ex) - g.cB[0] * (Ez[t + 1] - ez);
-  g.F[5][t] -= g.cB[0] * (Ey[t + 1] - ey) - g.cB[1] * (Ex[t + g.sy] - ex);
+  if constexpr (CKC) {
+    g.F[3][t] -= g.cB[1] * ckc_diff<R, 1>(g, Ez, t) - g.cB[2] * ckc_diff<R, 2>(g, Ey, t);
+    g.F[4][t] -= g.cB[2] * ckc_diff<R, 2>(g, Ex, t) - g.cB[0] * ckc_diff<R, 0>(g, Ez, t);
+    g.F[5][t] -= g.cB[0] * ckc_diff<R, 0>(g, Ey, t) - g.cB[1] * ckc_diff<R, 1>(g, Ex, t);
+  } else {
+    R ex = Ex[t], ey = Ey[t], ez = Ez[t];
+    g.F[3][t] -= g.cB[1] * (Ez[t + g.sy] - ez) - g.cB[2] * (Ey[t + g.sz] - ey);
+    g.F[4][t] -= g.cB[2] * (Ex[t + g.sz] - ex) - g.cB[0] * (Ez[t + 1] - ez);
+    g.F[5][t] -= g.cB[0] * (Ey[t + 1] - ey) - g.cB[1] * (Ex[t + g.sy] - ex);
+  }
 }
 
 // E += dt (c^2 curl B - J/eps0), backward differences
@@ -170,7 +189,8 @@ template <class R>
 void launch_push_B(const Grid<R>& g, const int lo[3], const int hi[3], Ctx& c) {
   Box3 b;
   for (int d = 0; d < 3; ++d) { b.lo[d] = lo[d]; b.n[d] = hi[d] - lo[d]; }
-  k_push_B<R><<<grd(b.n[0], b.n[1], b.n[2]), blk(), 0, c.stream>>>(g, b);
+  if (g.solver == 1) k_push_B<R, true><<<grd(b.n[0], b.n[1], b.n[2]), blk(), 0, c.stream>>>(g, b);
+  else k_push_B<R, false><<<grd(b.n[0], b.n[1], b.n[2]), blk(), 0, c.stream>>>(g, b);
   c.launches++;
 }
 template <class R>

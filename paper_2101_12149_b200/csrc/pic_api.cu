@@ -3,6 +3,7 @@
 // on one stream.
 #include "pic.h"
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -138,6 +139,22 @@ struct Sim : SimBase {
     g.dt = (R)dt_;
     g.pusher = o.pusher;
     g.gather_mode = o.gather_mode;
+    g.solver = o.solver;
+    {   // CKC weights: delta = min dx, r_a = (delta/dx_a)^2, S = r_y r_z + r_z r_x + r_x r_y
+      const double delta = std::min(dx_[0], std::min(dx_[1], dx_[2]));
+      double r[3];
+      for (int d = 0; d < 3; ++d) r[d] = (delta / dx_[d]) * (delta / dx_[d]);
+      const double S = r[1] * r[2] + r[2] * r[0] + r[0] * r[1];
+      const double beta = 0.125 * (1.0 - r[0] * r[1] * r[2] / S);
+      for (int a = 0; a < 3; ++a) {
+        const int b = (a + 1) % 3, cc = (a + 2) % 3;
+        const double bab = r[b] * beta, bac = r[cc] * beta;
+        const double ga = r[b] * r[cc] * (0.0625 - 0.125 * r[b] * r[cc] / S);
+        g.ck_b[a][a] = R(0); g.ck_b[a][b] = (R)bab; g.ck_b[a][cc] = (R)bac;
+        g.ck_g[a] = (R)ga;
+        g.ck_a[a] = (R)(1.0 - 2.0 * bab - 2.0 * bac - 4.0 * ga);
+      }
+    }
     // one allocation for the nine field arrays
     R* base = palloc<R>((size_t)tot * 9);
     if (!base) return fail(PIC_ERR_OOM, "field allocation failed");
@@ -348,9 +365,12 @@ struct Sim : SimBase {
     int loB[3], hiB[3], loE[3], hiE[3], lo0[3], hi0[3];
     for (int d = 0; d < 3; ++d) {
       lo0[d] = 0; hi0[d] = g.N[d];
-      loB[d] = g.periodic[d] ? -1 : 0;
-      hiB[d] = g.periodic[d] ? g.N[d] + 1 : g.N[d];
-      loE[d] = 0;
+      // Yee: the second B half-step reads E one layer up; CKC also reads one layer to every side, so its
+      // E update is widened to [-1, N+2) and its first B half-step to [-2, N+2) (guards are 4 deep)
+      const int wide = g.solver == PIC_SOLVER_CKC ? 2 : 1;
+      loB[d] = g.periodic[d] ? -wide : 0;
+      hiB[d] = g.periodic[d] ? g.N[d] + wide : g.N[d];
+      loE[d] = g.periodic[d] ? -(wide - 1) : 0;
       hiE[d] = hiB[d];
     }
     const int64_t launches0 = ctx.launches;
@@ -544,6 +564,7 @@ void pic_default_options(pic_options* o) {
   o->deposit_mode = PIC_DEPOSIT_AUTO;
   o->pusher = PIC_PUSHER_BORIS;
   o->gather_mode = PIC_GATHER_UNIFORM;
+  o->solver = PIC_SOLVER_YEE;
   o->cuda_stream = nullptr;
 }
 
@@ -559,8 +580,9 @@ int pic_create(const int32_t n_cells[3], const double dx[3], double dt, int shap
   if (opt) o = *opt;
   if (shape_order < 1 || shape_order > 3) return bad(PIC_ERR_INVALID_ARG, "shape_order must be 1, 2 or 3");
   if (prec != PIC_F64 && prec != PIC_F32) return bad(PIC_ERR_INVALID_ARG, "unknown precision");
-  if (o.sort_interval < 0 || o.sort_key_mode < 0 || o.sort_key_mode > 1 || o.reserved != 0 || o.deposit_mode < 0 ||
-      o.deposit_mode > 4 || o.pusher < 0 || o.pusher > 1 || o.gather_mode < 0 || o.gather_mode > 1)
+  if (o.sort_interval < 0 || o.sort_key_mode < 0 || o.sort_key_mode > 1 || o.deposit_mode < 0 ||
+      o.deposit_mode > 4 || o.pusher < 0 || o.pusher > 1 || o.gather_mode < 0 || o.gather_mode > 1 ||
+      o.solver < 0 || o.solver > 1)
     return bad(PIC_ERR_INVALID_ARG, "bad option value");
   double s2 = 0;
   for (int d = 0; d < 3; ++d) {
@@ -572,7 +594,10 @@ int pic_create(const int32_t n_cells[3], const double dx[3], double dt, int shap
     s2 += 1.0 / (dx[d] * dx[d]);
   }
   if (!(dt > 0) || !std::isfinite(dt)) return bad(PIC_ERR_INVALID_ARG, "dt must be positive and finite");
-  if (dt * kC * std::sqrt(s2) > 1.0) return bad(PIC_ERR_CFL, "dt violates the CFL limit dt*c*sqrt(sum 1/dx^2) <= 1");
+  if (o.solver == PIC_SOLVER_YEE && dt * kC * std::sqrt(s2) > 1.0)
+    return bad(PIC_ERR_CFL, "dt violates the CFL limit dt*c*sqrt(sum 1/dx^2) <= 1");
+  if (o.solver == PIC_SOLVER_CKC && dt * kC > std::min(dx[0], std::min(dx[1], dx[2])) * (1.0 + 1e-12))
+    return bad(PIC_ERR_CFL, "dt violates the CKC limit c*dt <= min(dx)");
   int ndev = 0;
   cudaError_t e = cudaGetDeviceCount(&ndev);
   if (e != cudaSuccess || ndev == 0) {

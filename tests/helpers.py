@@ -14,7 +14,7 @@ def make_pair(cfg, fields="config", shuffle=True, gpu_kwargs=None, with_oracle=T
     if fields == "random":
         E, B = W.random_fields(cfg, np.random.default_rng(rng_fields_seed))
     kw = dict(periodic=cfg.periodic, tile=cfg.tile, sort_interval=cfg.sort_interval)
-    kw.update(method or {})          # pusher= / gather_mode=, same values on both sides
+    kw.update(method or {})          # pusher= / gather_mode= / solver=, same values on both sides
     o = None
     if with_oracle:
         o = oracle.Oracle(cfg.n_cells, cfg.dx, cfg.dt, cfg.order, dtype=cfg.np_dtype, **kw)

@@ -39,7 +39,7 @@ def test_default_options(pic):
     o = pic.pic_default_options()
     assert list(o.periodic) == [1, 1, 1] and list(o.tile) == [8, 8, 8]
     assert o.sort_interval == 4 and o.sort_key_mode == 0 and o.deposit_mode == 0
-    assert o.pusher == 0 and o.gather_mode == 0 and o.reserved == 0
+    assert o.pusher == 0 and o.gather_mode == 0 and o.solver == 0
 
 
 def test_argument_errors_without_device(pic):

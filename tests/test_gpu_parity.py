@@ -147,6 +147,36 @@ def test_vay_and_galerkin_change_the_result():
         assert np.max(np.abs(g.get_particles(0)["ux"] - ub)) > 1e-11 * np.max(np.abs(ub))
 
 
+@pytest.mark.parametrize("periodic", [(1, 1, 1), (1, 1, 0)])
+def test_ckc_solver_matches_oracle(periodic):
+    """CKC field solver at c dt = 0.999 min(dx), beyond Yee's limit: fields only over
+    many steps, then the whole loop with particles (the widened guard-layer updates are exercised by the
+    periodic axes, the zero guards by the truncated one)."""
+    import oracle
+    import paper_2101_12149_b200 as pic
+    n, dx = (16, 12, 20), (1.0e-6, 0.8e-6, 0.5e-6)
+    dt = 0.999 * min(dx) / W.C_LIGHT
+    cfg = small("C2", n, order=3, dx=dx, tile=(4, 4, 4))
+    cfg.cfl = 0.999 * min(dx) * math.sqrt(sum(1.0 / (d * d) for d in dx))     # dt is derived from cfl
+    assert abs(cfg.dt - dt) < 1e-12 * dt
+    cfg.periodic = periodic
+    cfg.species[0].sigma = 0.2
+    with pytest.raises(pic.PicError):
+        pic.Sim(n, dx, dt, 3)                                  # Yee rejects this time step
+    import copy
+    cf = copy.deepcopy(cfg)
+    cf.species = []                                            # fields only
+    o, g, _ = make_pair(cf, fields="random", method=dict(solver=1))
+    o.step(25); g.step(25)
+    Eo, Bo, _ = o.get_fields(); Eg, Bg, _ = g.get_fields()
+    assert family_err(Eg, Eo) <= 50 * TOL64 and family_err(Bg, Bo) <= 50 * TOL64
+    o2, g2, _ = make_pair(cfg, fields="random", method=dict(solver=1))
+    o2.step(1); g2.step(1)
+    compare_state(o2, g2, TOL64)
+    o2.step(3); g2.step(3)
+    compare_state(o2, g2, 20 * TOL64)
+
+
 def test_vay_and_galerkin_fp32():
     cfg = small("C3", (16, 16, 16), order=3)
     cfg.species[0].sigma = 0.3
