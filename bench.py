@@ -247,6 +247,7 @@ def config_dict(cfg, world, args):
         "l2": "inputs larger than L2 (particle state %.2f GB per buffer vs 126 MB L2)" % (
             cfg.n_particles * (7 * (8 if cfg.dtype == "f64" else 4) + 8) / 1e9),
         "deposit_mode": args.deposit_mode,
+        "variant": {"pusher": args.pusher, "gather_mode": args.gather_mode, "solver": args.solver},
     }
 
 
@@ -289,7 +290,8 @@ def run_ours(args):
     n_cell = cfg.n_cells[0] * cfg.n_cells[1] * cfg.n_cells[2]
     stream = torch.cuda.current_stream()
     kw = dict(dtype=np_dt, periodic=cfg.periodic, tile=cfg.tile, sort_interval=cfg.sort_interval,
-              deposit_mode=args.deposit_mode, sort_key_mode=args.sort_key_mode, stream=stream.cuda_stream)
+              deposit_mode=args.deposit_mode, sort_key_mode=args.sort_key_mode, stream=stream.cuda_stream,
+              pusher=args.pusher, gather_mode=args.gather_mode, solver=args.solver)
 
     # ---------------- leg 1: state resident in HBM
     sim = pic.Sim(cfg.n_cells, cfg.dx, cfg.dt, cfg.order, **kw)
@@ -476,6 +478,9 @@ def main(argv=None):
     ap.add_argument("--tile", default=None, help="sweeps: cells per sort bin, e.g. 4,4,4")
     ap.add_argument("--sort-key-mode", type=int, default=0, help="sweeps: 0 cell key inside the tile, 1 tile only")
     ap.add_argument("--sigma", type=float, default=None, help="sweeps: thermal momentum spread u/c of every species")
+    ap.add_argument("--pusher", type=int, default=0, help="variants: PIC_PUSHER_* (0 Boris, 1 Vay)")
+    ap.add_argument("--gather-mode", type=int, default=0, help="variants: PIC_GATHER_* (0 uniform, 1 Galerkin)")
+    ap.add_argument("--solver", type=int, default=0, help="variants: PIC_SOLVER_* (0 Yee, 1 CKC)")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs: device-resident leg only")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs: do not time the oracle")
     ap.add_argument("--traffic", type=float, default=None,

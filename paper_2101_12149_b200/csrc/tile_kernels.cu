@@ -63,18 +63,19 @@ struct PushBox {
   static constexpr int MAXD = 256;   // drifted particles a CTA lists before it gathers them in line
 };
 
-template <class R, int ORDER>
+// NX, NY, NZ weights per axis: ORDER + 1, or ORDER along a staggered axis of the Galerkin gather
+template <class R, int ORDER, int NX = ORDER + 1, int NY = ORDER + 1, int NZ = ORDER + 1>
 __device__ __forceinline__ R interp_box(const R* __restrict__ F, int base, const R* wx, const R* wy, const R* wz) {
   constexpr int E = PushBox<ORDER>::EXT, SX = PushBox<ORDER>::SX;
   R acc = 0;
 #pragma unroll
-  for (int c = 0; c <= ORDER; ++c) {
+  for (int c = 0; c < NZ; ++c) {
     R accb = 0;
 #pragma unroll
-    for (int b = 0; b <= ORDER; ++b) {
+    for (int b = 0; b < NY; ++b) {
       R acca = 0;
 #pragma unroll
-      for (int a = 0; a <= ORDER; ++a) acca += wx[a] * F[base + SX * a + b + E * c];
+      for (int a = 0; a < NX; ++a) acca += wx[a] * F[base + SX * a + b + E * c];
       accb += wy[b] * acca;
     }
     acc += wz[c] * accb;
@@ -94,14 +95,20 @@ __device__ __forceinline__ void push_store(const Grid<R>& g, const Particles<R>&
   p.ux[t] = u[0]; p.uy[t] = u[1]; p.uz[t] = u[2];
 }
 
-// GENERIC = false: Boris pusher and uniform-order gather, fixed at compile time (the default and the
+// VAR 0: Boris pusher and uniform-order gather, fixed at compile time (the default and the benchmarked
+// path); VAR 2: Boris and the Galerkin gather, fixed at compile time (its staggered axes carry one weight
+// less, so it reads 288 box elements per particle instead of 384 at order 3); VAR 1: pusher and
+// gather variant read from the Grid (PIC_PUSHER_*, PIC_GATHER_*).
 // benchmarked path); true: pusher and gather variant read from the Grid (PIC_PUSHER_*, PIC_GATHER_*).
-template <class R, int ORDER, bool GENERIC>
+template <class R, int ORDER, int VAR>
 __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn,
                                                                    R* __restrict__ yn, R* __restrict__ zn,
                                                                    const int32_t* __restrict__ tile_start, TileSpec ts) {
   using PB = PushBox<ORDER>;
   constexpr int E = PB::EXT, SX = PB::SX, VOL = PB::VOL;
+  constexpr bool GENERIC = VAR == 1;
+  constexpr int NS = VAR == 2 ? ORDER : ORDER + 1;   // weights along a staggered axis
+  constexpr int NN = ORDER + 1;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   R* box = reinterpret_cast<R*>(smem_raw);   // [6][E (x)][SX: E (z) x E (y), padded]
   __shared__ int s_drift[PB::MAXD];
@@ -146,7 +153,7 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
     for (int d = 0; d < 3; ++d) {
       R xi = x0[d] * g.inv_dx[d];
       ln[d] = shape<R, ORDER>(xi, wn[d]) - (d == 0 ? o0 : (d == 1 ? o1 : o2));
-      ls[d] = ((GENERIC && g.gather_mode) ? shape_lowered<R, ORDER>(xi - R(0.5), ws[d])
+      ls[d] = ((VAR == 2 || (GENERIC && g.gather_mode)) ? shape_lowered<R, ORDER>(xi - R(0.5), ws[d])
                                          : shape<R, ORDER>(xi - R(0.5), ws[d])) -
               (d == 0 ? o0 : (d == 1 ? o1 : o2));
       inbox &= (ln[d] >= 0) & (ln[d] <= E - ORDER - 1) & (ls[d] >= 0) & (ls[d] <= E - ORDER - 1);
@@ -157,18 +164,18 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
       const int slot = atomicAdd(&s_ndrift, 1);
       if (slot < PB::MAXD) { s_drift[slot] = t; continue; }
       R Ef[3], Bf[3];
-      gather6<R, ORDER, GENERIC>(g, x0[0], x0[1], x0[2], Ef, Bf);
+      gather6<R, ORDER, VAR != 0>(g, x0[0], x0[1], x0[2], Ef, Bf);
       push_store<R, GENERIC>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
       continue;
     }
     R Ef[3], Bf[3];
     // Ex (s,n,n)  Ey (n,s,n)  Ez (n,n,s)  Bx (n,s,s)  By (s,n,s)  Bz (s,s,n)
-    Ef[0] = interp_box<R, ORDER>(box + 0 * VOL, SX * ls[0] + ln[1] + E * ln[2], ws[0], wn[1], wn[2]);
-    Ef[1] = interp_box<R, ORDER>(box + 1 * VOL, SX * ln[0] + ls[1] + E * ln[2], wn[0], ws[1], wn[2]);
-    Ef[2] = interp_box<R, ORDER>(box + 2 * VOL, SX * ln[0] + ln[1] + E * ls[2], wn[0], wn[1], ws[2]);
-    Bf[0] = interp_box<R, ORDER>(box + 3 * VOL, SX * ln[0] + ls[1] + E * ls[2], wn[0], ws[1], ws[2]);
-    Bf[1] = interp_box<R, ORDER>(box + 4 * VOL, SX * ls[0] + ln[1] + E * ls[2], ws[0], wn[1], ws[2]);
-    Bf[2] = interp_box<R, ORDER>(box + 5 * VOL, SX * ls[0] + ls[1] + E * ln[2], ws[0], ws[1], wn[2]);
+    Ef[0] = interp_box<R, ORDER, NS, NN, NN>(box + 0 * VOL, SX * ls[0] + ln[1] + E * ln[2], ws[0], wn[1], wn[2]);
+    Ef[1] = interp_box<R, ORDER, NN, NS, NN>(box + 1 * VOL, SX * ln[0] + ls[1] + E * ln[2], wn[0], ws[1], wn[2]);
+    Ef[2] = interp_box<R, ORDER, NN, NN, NS>(box + 2 * VOL, SX * ln[0] + ln[1] + E * ls[2], wn[0], wn[1], ws[2]);
+    Bf[0] = interp_box<R, ORDER, NN, NS, NS>(box + 3 * VOL, SX * ln[0] + ls[1] + E * ls[2], wn[0], ws[1], ws[2]);
+    Bf[1] = interp_box<R, ORDER, NS, NN, NS>(box + 4 * VOL, SX * ls[0] + ln[1] + E * ls[2], ws[0], wn[1], ws[2]);
+    Bf[2] = interp_box<R, ORDER, NS, NS, NN>(box + 5 * VOL, SX * ls[0] + ls[1] + E * ln[2], ws[0], ws[1], wn[2]);
     push_store<R, GENERIC>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
   }
   __syncthreads();
@@ -178,7 +185,7 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
     R x0[3] = {p.x[t], p.y[t], p.z[t]};
     R u[3] = {p.ux[t], p.uy[t], p.uz[t]};
     R Ef[3], Bf[3];
-    gather6<R, ORDER, GENERIC>(g, x0[0], x0[1], x0[2], Ef, Bf);
+    gather6<R, ORDER, VAR != 0>(g, x0[0], x0[1], x0[2], Ef, Bf);
     push_store<R, GENERIC>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
   }
 }
@@ -735,8 +742,9 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, bool m
   const size_t vec_smem = (size_t)kW * 32 * TWin<ORDER>::REC * sizeof(R);
   const size_t mma_smem = (size_t)mw * 33 * MWin<ORDER>::REC * sizeof(R);
   if (!attr_set) {
-    cudaFuncSetAttribute(k_push_tile<R, ORDER, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
-    cudaFuncSetAttribute(k_push_tile<R, ORDER, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
+    cudaFuncSetAttribute(k_push_tile<R, ORDER, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
+    cudaFuncSetAttribute(k_push_tile<R, ORDER, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
+    cudaFuncSetAttribute(k_push_tile<R, ORDER, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
     cudaFuncSetAttribute(kvec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vec_smem);
     cudaFuncSetAttribute(kmma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mma_smem);
     attr_set = true;
@@ -744,11 +752,11 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, bool m
   {
     ScopedPhase ph(c, kPhasePush);
     if (g.pusher == 0 && g.gather_mode == 0)
-      k_push_tile<R, ORDER, false><<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start,
-                                                                                     a.tiles);
+      k_push_tile<R, ORDER, 0><<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles);
+    else if (g.pusher == 0 && g.gather_mode == 1)
+      k_push_tile<R, ORDER, 2><<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles);
     else
-      k_push_tile<R, ORDER, true><<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start,
-                                                                                    a.tiles);
+      k_push_tile<R, ORDER, 1><<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles);
   }
   {
     ScopedPhase ph(c, kPhaseDeposit);
