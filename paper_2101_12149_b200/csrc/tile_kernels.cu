@@ -83,11 +83,11 @@ __device__ __forceinline__ R interp_box(const R* __restrict__ F, int base, const
   return acc;
 }
 
-template <class R, bool GENERIC>
+template <class R, int PUSHER>
 __device__ __forceinline__ void push_store(const Grid<R>& g, const Particles<R>& p, R* __restrict__ xn,
                                            R* __restrict__ yn, R* __restrict__ zn, int t, const R* x0, R* u,
                                            const R* Ef, const R* Bf) {
-  push_momentum<R>(GENERIC ? g.pusher : 0, p.kq, g.inv_c2, Ef, Bf, u);
+  push_momentum<R>(PUSHER, p.kq, g.inv_c2, Ef, Bf, u);   // compile-time constant: the other branch folds away
   R ig = g.dt / sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * g.inv_c2);
   xn[t] = x0[0] + u[0] * ig;
   yn[t] = x0[1] + u[1] * ig;
@@ -95,19 +95,17 @@ __device__ __forceinline__ void push_store(const Grid<R>& g, const Particles<R>&
   p.ux[t] = u[0]; p.uy[t] = u[1]; p.uz[t] = u[2];
 }
 
-// VAR 0: Boris pusher and uniform-order gather, fixed at compile time (the default and the benchmarked
-// path); VAR 2: Boris and the Galerkin gather, fixed at compile time (its staggered axes carry one weight
-// less, so it reads 288 box elements per particle instead of 384 at order 3); VAR 1: pusher and
-// gather variant read from the Grid (PIC_PUSHER_*, PIC_GATHER_*).
-// benchmarked path); true: pusher and gather variant read from the Grid (PIC_PUSHER_*, PIC_GATHER_*).
-template <class R, int ORDER, int VAR>
+// Pusher (PIC_PUSHER_*) and gather variant (PIC_GATHER_*) are template parameters: four instantiations
+// per order and precision, (0, 0) being the default and benchmarked path. The Galerkin gather carries one
+// weight less along every staggered axis, so it reads 288 box elements per particle instead of 384 at
+// order 3 — and runs faster by that ratio, since those reads are what bounds the kernel.
+template <class R, int ORDER, int PUSHER, int GATHER>
 __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn,
                                                                    R* __restrict__ yn, R* __restrict__ zn,
                                                                    const int32_t* __restrict__ tile_start, TileSpec ts) {
   using PB = PushBox<ORDER>;
   constexpr int E = PB::EXT, SX = PB::SX, VOL = PB::VOL;
-  constexpr bool GENERIC = VAR == 1;
-  constexpr int NS = VAR == 2 ? ORDER : ORDER + 1;   // weights along a staggered axis
+  constexpr int NS = GATHER == 1 ? ORDER : ORDER + 1;   // weights along a staggered axis
   constexpr int NN = ORDER + 1;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   R* box = reinterpret_cast<R*>(smem_raw);   // [6][E (x)][SX: E (z) x E (y), padded]
@@ -153,7 +151,7 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
     for (int d = 0; d < 3; ++d) {
       R xi = x0[d] * g.inv_dx[d];
       ln[d] = shape<R, ORDER>(xi, wn[d]) - (d == 0 ? o0 : (d == 1 ? o1 : o2));
-      ls[d] = ((VAR == 2 || (GENERIC && g.gather_mode)) ? shape_lowered<R, ORDER>(xi - R(0.5), ws[d])
+      ls[d] = (GATHER == 1 ? shape_lowered<R, ORDER>(xi - R(0.5), ws[d])
                                          : shape<R, ORDER>(xi - R(0.5), ws[d])) -
               (d == 0 ? o0 : (d == 1 ? o1 : o2));
       inbox &= (ln[d] >= 0) & (ln[d] <= E - ORDER - 1) & (ls[d] >= 0) & (ls[d] <= E - ORDER - 1);
@@ -164,8 +162,8 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
       const int slot = atomicAdd(&s_ndrift, 1);
       if (slot < PB::MAXD) { s_drift[slot] = t; continue; }
       R Ef[3], Bf[3];
-      gather6<R, ORDER, VAR != 0>(g, x0[0], x0[1], x0[2], Ef, Bf);
-      push_store<R, GENERIC>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
+      gather6<R, ORDER, GATHER != 0>(g, x0[0], x0[1], x0[2], Ef, Bf);
+      push_store<R, PUSHER>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
       continue;
     }
     R Ef[3], Bf[3];
@@ -176,7 +174,7 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
     Bf[0] = interp_box<R, ORDER, NN, NS, NS>(box + 3 * VOL, SX * ln[0] + ls[1] + E * ls[2], wn[0], ws[1], ws[2]);
     Bf[1] = interp_box<R, ORDER, NS, NN, NS>(box + 4 * VOL, SX * ls[0] + ln[1] + E * ls[2], ws[0], wn[1], ws[2]);
     Bf[2] = interp_box<R, ORDER, NS, NS, NN>(box + 5 * VOL, SX * ls[0] + ls[1] + E * ln[2], ws[0], ws[1], wn[2]);
-    push_store<R, GENERIC>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
+    push_store<R, PUSHER>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
   }
   __syncthreads();
   const int nd = min(s_ndrift, PB::MAXD);
@@ -185,8 +183,8 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
     R x0[3] = {p.x[t], p.y[t], p.z[t]};
     R u[3] = {p.ux[t], p.uy[t], p.uz[t]};
     R Ef[3], Bf[3];
-    gather6<R, ORDER, VAR != 0>(g, x0[0], x0[1], x0[2], Ef, Bf);
-    push_store<R, GENERIC>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
+    gather6<R, ORDER, GATHER != 0>(g, x0[0], x0[1], x0[2], Ef, Bf);
+    push_store<R, PUSHER>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
   }
 }
 
@@ -742,21 +740,19 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, bool m
   const size_t vec_smem = (size_t)kW * 32 * TWin<ORDER>::REC * sizeof(R);
   const size_t mma_smem = (size_t)mw * 33 * MWin<ORDER>::REC * sizeof(R);
   if (!attr_set) {
-    cudaFuncSetAttribute(k_push_tile<R, ORDER, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
-    cudaFuncSetAttribute(k_push_tile<R, ORDER, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
-    cudaFuncSetAttribute(k_push_tile<R, ORDER, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
+    cudaFuncSetAttribute(k_push_tile<R, ORDER, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
+    cudaFuncSetAttribute(k_push_tile<R, ORDER, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
+    cudaFuncSetAttribute(k_push_tile<R, ORDER, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
+    cudaFuncSetAttribute(k_push_tile<R, ORDER, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
     cudaFuncSetAttribute(kvec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vec_smem);
     cudaFuncSetAttribute(kmma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mma_smem);
     attr_set = true;
   }
   {
     ScopedPhase ph(c, kPhasePush);
-    if (g.pusher == 0 && g.gather_mode == 0)
-      k_push_tile<R, ORDER, 0><<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles);
-    else if (g.pusher == 0 && g.gather_mode == 1)
-      k_push_tile<R, ORDER, 2><<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles);
-    else
-      k_push_tile<R, ORDER, 1><<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles);
+    auto kpush = g.pusher == 0 ? (g.gather_mode == 0 ? k_push_tile<R, ORDER, 0, 0> : k_push_tile<R, ORDER, 0, 1>)
+                               : (g.gather_mode == 0 ? k_push_tile<R, ORDER, 1, 0> : k_push_tile<R, ORDER, 1, 1>);
+    kpush<<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles);
   }
   {
     ScopedPhase ph(c, kPhaseDeposit);
