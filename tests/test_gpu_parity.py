@@ -177,6 +177,26 @@ def test_ckc_solver_matches_oracle(periodic):
     compare_state(o2, g2, 20 * TOL64)
 
 
+def test_C1_twenty_steps_with_vay_galerkin_ckc():
+    """BASELINE.json config 1 in full with all three method variants switched on: aggregates after 20 steps
+    (5 sorts) within 1e-3 of the oracle's, charge exact, Gauss residual constant, particles by id."""
+    cfg = W.CONFIGS["C1"]
+    o, g, _ = make_pair(cfg, method=dict(pusher=1, gather_mode=1, solver=1))
+    d0 = g.diagnostics()
+    o.step(cfg.steps); g.step(cfg.steps)
+    do, dg = o.diagnostics(), g.diagnostics()
+    eo = do["field_E"] + do["field_B"] + do["kinetic"]
+    eg = dg["field_E"] + dg["field_B"] + dg["kinetic"]
+    assert abs(eg - eo) < 1e-3 * eo
+    assert abs(dg["field_E"] - do["field_E"]) < 1e-3 * do["field_E"]
+    assert dg["charge"] == pytest.approx(d0["charge"], rel=1e-12)
+    assert abs(dg["gauss_max"] - d0["gauss_max"]) < 1e-9 * d0["rho_max"]
+    po, pg = o.get_particles(), g.get_particles()
+    io, ig = np.argsort(po["id"]), np.argsort(pg["id"])
+    for k in ("x", "ux"):
+        assert np.max(np.abs(po[k][io] - pg[k][ig])) < 1e-9 * np.max(np.abs(po[k]))
+
+
 def test_vay_and_galerkin_fp32():
     cfg = small("C3", (16, 16, 16), order=3)
     cfg.species[0].sigma = 0.3
