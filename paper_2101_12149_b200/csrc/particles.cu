@@ -377,7 +377,7 @@ bool launch_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) 
     cudaMemsetAsync(a.stray_count, 0, 2 * sizeof(unsigned int), c.stream);
     launch_tile_kernels<R>(g, a, ORDER, mode == kDepositTileMma, c);
     ScopedPhase ph(c, kPhaseStray);
-    k_deposit_list_warp<R, ORDER><<<148 * 16, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count,
+    k_deposit_list_warp<R, ORDER><<<148 * 64, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count,
                                                                  a.deactivated);
     c.launches += 1;
     return true;
