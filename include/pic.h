@@ -209,6 +209,14 @@ PIC_API int32_t pic_num_species(const pic_sim* sim);
  * The string is owned by the library and valid until the next call on the same handle. */
 PIC_API const char* pic_last_error(const pic_sim* sim);
 
+/* The weights the CKC solver (PIC_SOLVER_CKC, ref [12]) uses for cells of size dx[3]: the difference of
+ * E along axis a in the B update is alpha[a]*dF(0,0) + beta[3a+b]*[dF(+b) + dF(-b)] + beta[3a+c]*[dF(+c) +
+ * dF(-c)] + gamma[a]*[the four corners] over the 3x3 transverse neighbours (b, c the other two axes;
+ * beta[3a+a] = 0). Host arithmetic only, no device needed (lets the weights be checked against what they
+ * are built for: unit sum, stability at c*dt = min(dx), no dispersion along the axes). Host pointers:
+ * alpha[3], beta[9], gamma[3]. Errors: INVALID_ARG. */
+PIC_API int pic_ckc_coefficients(const double dx[3], double alpha[3], double beta[9], double gamma[3]);
+
 /* Free everything the handle owns (synchronises). NULL is a no-op. */
 PIC_API void pic_destroy(pic_sim* sim);
 

@@ -31,7 +31,7 @@ SYMBOLS = (
     "pic_default_options", "pic_create", "pic_add_species", "pic_set_fields", "pic_step", "pic_synchronize",
     "pic_get_fields", "pic_get_particles", "pic_get_sort_state", "pic_sort_now", "pic_get_diagnostics",
     "pic_get_rho", "pic_enable_phase_timing", "pic_get_phase_times", "pic_num_particles", "pic_num_species",
-    "pic_last_error", "pic_destroy",
+    "pic_last_error", "pic_ckc_coefficients", "pic_destroy",
 )
 
 
@@ -82,6 +82,7 @@ def lib():
         L.pic_num_species.restype = C.c_int32
         L.pic_last_error.argtypes = [vp]
         L.pic_last_error.restype = C.c_char_p
+        L.pic_ckc_coefficients.argtypes = [dp, dp, dp, dp]
         L.pic_destroy.argtypes = [vp]
         L.pic_destroy.restype = None
         _lib = L
@@ -218,6 +219,15 @@ def pic_num_particles(h, species=0) -> int:
 
 def pic_num_species(h) -> int:
     return lib().pic_num_species(h)
+
+
+def pic_ckc_coefficients(dx):
+    """(alpha[3], beta[3][3], gamma[3]) of the CKC solver for cells of size dx (host arithmetic only)."""
+    al, be, ga = (C.c_double * 3)(), (C.c_double * 9)(), (C.c_double * 3)()
+    rc = lib().pic_ckc_coefficients((C.c_double * 3)(*[float(v) for v in dx]), al, be, ga)
+    if rc != 0:
+        raise PicError(rc, "dx must be positive and finite")
+    return np.array(al[:]), np.array(be[:]).reshape(3, 3), np.array(ga[:])
 
 
 def pic_destroy(h):

@@ -27,6 +27,30 @@ __global__ void k_iota(int64_t* p, int64_t n) {
   if (t < n) p[t] = t;
 }
 
+// Weights of the CKC smoothed differences (include/pic.h, pic_ckc_coefficients), written in the inverse
+// square spacings k_a = 1/dx_a^2 with d2 = min(dx)^2 = 1/max(k): for the difference along a, with b and c
+// the transverse axes and Q = k_x k_y + k_y k_z + k_z k_x,
+//   beta_ab = d2 k_b (1 - d2 k_x k_y k_z / Q) / 8,   gamma_a = d2^2 k_b k_c (1/16 - k_b k_c / (8 Q)),
+//   alpha_a = 1 - 2 beta_ab - 2 beta_ac - 4 gamma_a.
+// Pinned on this side by tests/test_abi.py (cubic 7/12, 1/12, 1/48; unit sum; the von Neumann bound at
+// c dt = min dx; no dispersion along an axis), independently of the oracle's own copy of the scheme.
+void ckc_weights(const double* dx, double* alpha, double (*beta)[3], double* gamma) {
+  const double k[3] = {1.0 / (dx[0] * dx[0]), 1.0 / (dx[1] * dx[1]), 1.0 / (dx[2] * dx[2])};
+  const double d2 = 1.0 / std::max(k[0], std::max(k[1], k[2]));
+  const double Q = k[0] * k[1] + k[1] * k[2] + k[2] * k[0];
+  const double common = (1.0 - d2 * (k[0] * k[1] * k[2]) / Q) / 8.0;
+  for (int a = 0; a < 3; ++a) {
+    double two_beta = 0.0, kk = 1.0;
+    for (int b = 0; b < 3; ++b) {
+      beta[a][b] = b == a ? 0.0 : d2 * k[b] * common;
+      two_beta += 2.0 * beta[a][b];
+      if (b != a) kk *= k[b];
+    }
+    gamma[a] = d2 * d2 * kk * (1.0 / 16.0 - kk / (8.0 * Q));
+    alpha[a] = 1.0 - two_beta - 4.0 * gamma[a];
+  }
+}
+
 struct SimBase {
   virtual ~SimBase() {}
   std::string err;
@@ -140,19 +164,13 @@ struct Sim : SimBase {
     g.pusher = o.pusher;
     g.gather_mode = o.gather_mode;
     g.solver = o.solver;
-    {   // CKC weights: delta = min dx, r_a = (delta/dx_a)^2, S = r_y r_z + r_z r_x + r_x r_y
-      const double delta = std::min(dx_[0], std::min(dx_[1], dx_[2]));
-      double r[3];
-      for (int d = 0; d < 3; ++d) r[d] = (delta / dx_[d]) * (delta / dx_[d]);
-      const double S = r[1] * r[2] + r[2] * r[0] + r[0] * r[1];
-      const double beta = 0.125 * (1.0 - r[0] * r[1] * r[2] / S);
+    {
+      double al[3], be[3][3], ga[3];
+      ckc_weights(dx_, al, be, ga);
       for (int a = 0; a < 3; ++a) {
-        const int b = (a + 1) % 3, cc = (a + 2) % 3;
-        const double bab = r[b] * beta, bac = r[cc] * beta;
-        const double ga = r[b] * r[cc] * (0.0625 - 0.125 * r[b] * r[cc] / S);
-        g.ck_b[a][a] = R(0); g.ck_b[a][b] = (R)bab; g.ck_b[a][cc] = (R)bac;
-        g.ck_g[a] = (R)ga;
-        g.ck_a[a] = (R)(1.0 - 2.0 * bab - 2.0 * bac - 4.0 * ga);
+        g.ck_a[a] = (R)al[a];
+        g.ck_g[a] = (R)ga[a];
+        for (int b = 0; b < 3; ++b) g.ck_b[a][b] = (R)be[a][b];
       }
     }
     // one allocation for the nine field arrays
@@ -707,6 +725,17 @@ int32_t pic_num_species(const pic_sim* sim) {
 const char* pic_last_error(const pic_sim* sim) {
   if (!sim || !sim->impl) return pic::g_create_error.c_str();
   return sim->impl->err.c_str();
+}
+
+int pic_ckc_coefficients(const double dx[3], double alpha[3], double beta[9], double gamma[3]) {
+  if (!dx || !alpha || !beta || !gamma) return PIC_ERR_INVALID_ARG;
+  for (int d = 0; d < 3; ++d)
+    if (!(dx[d] > 0) || !std::isfinite(dx[d])) return PIC_ERR_INVALID_ARG;
+  double be[3][3];
+  pic::ckc_weights(dx, alpha, be, gamma);
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b) beta[3 * a + b] = be[a][b];
+  return PIC_OK;
 }
 
 void pic_destroy(pic_sim* sim) {

@@ -93,3 +93,39 @@ def test_product_does_not_import_oracle():
     orc = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "pic_oracle.cpp")).read()
     assert "import paper_2101_12149_b200" not in orc and "libpic" not in orc and "csrc/" not in orc.replace(
         "paper_2101_12149_b200/csrc", "")
+
+
+def test_ckc_weights_of_the_product_do_what_they_are_built_for(pic):
+    """The CUDA side's own CKC weights (pic_ckc_coefficients, host arithmetic, written in the inverse square
+    spacings) against what fixes them, with no reference to the oracle's copy: the published cubic-cell
+    values 7/12, 1/12, 1/48 (ref [12]); every smoothed difference sums to 1; with c dt = min(dx) the von
+    Neumann bound 0 <= (c dt)^2 sum_a S_a sin^2(k_a dx_a/2)/dx_a^2 <= 1 holds for every wave vector and is
+    reached; a wave along the finest axis has no dispersion at that time step."""
+    import math
+    c = 299792458.0
+    al, be, ga = pic.pic_ckc_coefficients((1e-6,) * 3)
+    assert np.allclose(al, 7 / 12, rtol=1e-15) and np.allclose(ga, 1 / 48, rtol=1e-14)
+    assert np.allclose(be[~np.eye(3, dtype=bool)], 1 / 12, rtol=1e-14) and np.all(np.diag(be) == 0)
+    for dx in [(1e-6, 1e-6, 1e-6), (1e-6, 0.8e-6, 0.5e-6), (0.1e-6, 0.1e-6, 0.025e-6), (2e-6, 1e-6, 1e-6)]:
+        al, be, ga = pic.pic_ckc_coefficients(dx)
+        dt = min(dx) / c
+        for a in range(3):
+            b, cc = (a + 1) % 3, (a + 2) % 3
+            assert abs(al[a] + 2 * be[a][b] + 2 * be[a][cc] + 4 * ga[a] - 1) < 1e-15
+        th = np.linspace(0, math.pi, 25)
+        cx, cy, cz = np.meshgrid(np.cos(th), np.cos(th), np.cos(th), indexing="ij")
+        sx, sy, sz = np.meshgrid(np.sin(th / 2) ** 2, np.sin(th / 2) ** 2, np.sin(th / 2) ** 2, indexing="ij")
+        cs, s2 = (cx, cy, cz), (sx, sy, sz)
+        tot = 0.0
+        for a in range(3):
+            b, cc = (a + 1) % 3, (a + 2) % 3
+            S = al[a] + 2 * be[a][b] * cs[b] + 2 * be[a][cc] * cs[cc] + 4 * ga[a] * cs[b] * cs[cc]
+            tot = tot + S * s2[a] / dx[a] ** 2
+        tot = tot * (c * dt) ** 2
+        assert tot.min() > -1e-14 and tot.max() <= 1 + 1e-12 and tot.max() > 0.999
+        # along the finest axis alone: S = 1, so sin^2(omega dt/2) = sin^2(k dx/2), i.e. omega = c k
+        a = int(np.argmin(dx))
+        b, cc = (a + 1) % 3, (a + 2) % 3
+        assert abs(al[a] + 2 * be[a][b] + 2 * be[a][cc] + 4 * ga[a] - 1) < 1e-15
+    with pytest.raises(pic.PicError):
+        pic.pic_ckc_coefficients((1e-6, 0.0, 1e-6))
