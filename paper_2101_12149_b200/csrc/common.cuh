@@ -47,11 +47,60 @@ struct TileSpec {
   int key_mode;  // 0 tile-major cell key, 1 tile only
 };
 
+// ------------------------------------------------------------------ rounded arithmetic
+// Operations the compiler may neither contract into an FMA nor reassociate. mul_rn: the one rounded
+// multiply of the sort rule and of every normalised coordinate xi = x * inv_dx.
+// sub_rn: difference of two ROUNDED values (DS = S1 - S0 cancels to roundoff for a slow particle).
+// In fp32 the whole chain position -> weights -> gathered field -> momentum -> new position is written
+// with them in the operation order of the method's statement (left to
+// right), so that x_new and u_new come out bit for bit what that statement gives in IEEE single
+// precision: one fp32 ulp of a position is 1e-3 of a step's displacement at 128 cells, and the
+// deposit's DS = S1 - S0 would otherwise carry that into J.
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ double sub_rn(double a, double b) { return __dsub_rn(a, b); }
+__device__ __forceinline__ float sub_rn(float a, float b) { return __fsub_rn(a, b); }
+__device__ __forceinline__ double add_rn(double a, double b) { return __dadd_rn(a, b); }
+__device__ __forceinline__ float add_rn(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ double div_rn(double a, double b) { return __ddiv_rn(a, b); }
+__device__ __forceinline__ float div_rn(float a, float b) { return __fdiv_rn(a, b); }
+__device__ __forceinline__ double sqrt_rn(double a) { return __dsqrt_rn(a); }
+__device__ __forceinline__ float sqrt_rn(float a) { return __fsqrt_rn(a); }
+// fp32: statement order, every operation rounded; fp64: the compiler's contractions are welcome
+// (they only add accuracy, and 1e-12 leaves room for them)
+template <class R> constexpr bool kStatementOrder = sizeof(R) == 4;
+
 // ------------------------------------------------------------------ shape factors
 // B-spline weights of order n at normalised coordinate xi; returns the leftmost node index.
 template <class R, int ORDER>
 __device__ __forceinline__ int shape(R xi, R* w) {
-  if constexpr (ORDER == 1) {
+  if constexpr (kStatementOrder<R>) {
+    const R h = R(0.5);
+    if constexpr (ORDER == 1) {
+      R m = floor(xi);
+      R d = sub_rn(xi, m);
+      w[0] = sub_rn(R(1), d);
+      w[1] = d;
+      return (int)m;
+    } else if constexpr (ORDER == 2) {
+      R m = floor(add_rn(xi, h));
+      R d = sub_rn(xi, m);
+      R a = sub_rn(h, d), b = add_rn(h, d);
+      w[0] = mul_rn(mul_rn(h, a), a);
+      w[1] = sub_rn(R(0.75), mul_rn(d, d));
+      w[2] = mul_rn(mul_rn(h, b), b);
+      return (int)m - 1;
+    } else {
+      R m = floor(xi);
+      R d = sub_rn(xi, m);
+      R e = sub_rn(R(1), d);
+      w[0] = div_rn(mul_rn(mul_rn(e, e), e), R(6));
+      w[1] = div_rn(add_rn(sub_rn(R(4), mul_rn(mul_rn(R(6), d), d)), mul_rn(mul_rn(mul_rn(R(3), d), d), d)), R(6));
+      w[2] = div_rn(add_rn(sub_rn(R(4), mul_rn(mul_rn(R(6), e), e)), mul_rn(mul_rn(mul_rn(R(3), e), e), e)), R(6));
+      w[3] = div_rn(mul_rn(mul_rn(d, d), d), R(6));
+      return (int)m - 1;
+    }
+  } else if constexpr (ORDER == 1) {
     R m = floor(xi);
     R d = xi - m;
     w[0] = R(1) - d;
@@ -85,20 +134,11 @@ __device__ __forceinline__ int shape_lowered(R xi, R* w) {
   w[ORDER] = R(0);
   if constexpr (ORDER == 1) {            // order 0: nearest grid point
     w[0] = R(1);
-    return (int)floor(xi + R(0.5));
+    return (int)floor(add_rn(xi, R(0.5)));
   } else {
     return shape<R, ORDER - 1>(xi, w);
   }
 }
-
-// one rounded multiply, no FMA contraction
-__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
-__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
-
-// difference of two ROUNDED values: keeps the compiler from contracting the last multiply of a
-// shape weight into the subtraction (DS = S1 - S0 cancels to roundoff for a slow particle)
-__device__ __forceinline__ double sub_rn(double a, double b) { return __dsub_rn(a, b); }
-__device__ __forceinline__ float sub_rn(float a, float b) { return __fsub_rn(a, b); }
 
 template <class R>
 __device__ __forceinline__ int cell_of(R x, R inv_dx, int N) {

@@ -102,7 +102,7 @@ __global__ void __launch_bounds__(128) k_rho(Grid<R> g, Particles<R> p, double q
   int l[3];
   R pos[3] = {p.x[t], p.y[t], p.z[t]};
 #pragma unroll
-  for (int d = 0; d < 3; ++d) l[d] = shape<R, ORDER>(pos[d] * g.inv_dx[d], w[d]);
+  for (int d = 0; d < 3; ++d) l[d] = shape<R, ORDER>(mul_rn(pos[d], g.inv_dx[d]), w[d]);
   double inv_dv = (double)g.inv_dx[0] * (double)g.inv_dx[1] * (double)g.inv_dx[2];
   double qw = q * (double)p.w[t] * inv_dv;
 #pragma unroll

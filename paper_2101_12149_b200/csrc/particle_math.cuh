@@ -12,6 +12,16 @@ template <class R, int ORDER>
 __device__ __forceinline__ R interp(const R* __restrict__ F, int base, int sy, int sz,
                                     const R* wx, const R* wy, const R* wz) {
   R acc = 0;
+  if constexpr (kStatementOrder<R>) {   // sum over c, b, a (a innermost) of ((wx wy) wz) F, every operation rounded
+#pragma unroll
+    for (int c = 0; c <= ORDER; ++c)
+#pragma unroll
+      for (int b = 0; b <= ORDER; ++b)
+#pragma unroll
+        for (int a = 0; a <= ORDER; ++a)
+          acc = add_rn(acc, mul_rn(mul_rn(mul_rn(wx[a], wy[b]), wz[c]), __ldg(F + base + a + sy * b + sz * c)));
+    return acc;
+  }
 #pragma unroll
   for (int c = 0; c <= ORDER; ++c) {
     R accb = 0;
@@ -35,10 +45,10 @@ __device__ __forceinline__ void gather6(const Grid<R>& g, R x, R y, R z, R* E, R
   R pos[3] = {x, y, z};
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
-    R xi = pos[d] * g.inv_dx[d];
+    const R xi = mul_rn(pos[d], g.inv_dx[d]);
+    const R xs = sub_rn(xi, R(0.5));
     ln[d] = shape<R, ORDER>(xi, wn[d]);
-    ls[d] = (GENERIC && g.gather_mode) ? shape_lowered<R, ORDER>(xi - R(0.5), ws[d])
-                                       : shape<R, ORDER>(xi - R(0.5), ws[d]);
+    ls[d] = (GENERIC && g.gather_mode) ? shape_lowered<R, ORDER>(xs, ws[d]) : shape<R, ORDER>(xs, ws[d]);
     // memory safety if a position ever went non-finite: keep the stencil inside the padded box
     ln[d] = min(max(ln[d], -kGuard), g.N[d] + kGuard - ORDER - 1);
     ls[d] = min(max(ls[d], -kGuard), g.N[d] + kGuard - ORDER - 1);
@@ -56,6 +66,27 @@ __device__ __forceinline__ void gather6(const Grid<R>& g, R x, R y, R z, R* E, R
 // ------------------------------------------------------------------ Boris
 template <class R>
 __device__ __forceinline__ void boris(R kq, R inv_c2, const R* E, const R* B, R* u) {
+  if constexpr (kStatementOrder<R>) {
+    R um[3], t[3], up[3], sv[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) um[d] = add_rn(u[d], mul_rn(kq, E[d]));
+    const R g = sqrt_rn(add_rn(R(1), mul_rn(add_rn(add_rn(mul_rn(um[0], um[0]), mul_rn(um[1], um[1])), mul_rn(um[2], um[2])), inv_c2)));
+#pragma unroll
+    for (int d = 0; d < 3; ++d) t[d] = div_rn(mul_rn(kq, B[d]), g);
+    up[0] = add_rn(um[0], sub_rn(mul_rn(um[1], t[2]), mul_rn(um[2], t[1])));
+    up[1] = add_rn(um[1], sub_rn(mul_rn(um[2], t[0]), mul_rn(um[0], t[2])));
+    up[2] = add_rn(um[2], sub_rn(mul_rn(um[0], t[1]), mul_rn(um[1], t[0])));
+    const R den = add_rn(R(1), add_rn(add_rn(mul_rn(t[0], t[0]), mul_rn(t[1], t[1])), mul_rn(t[2], t[2])));
+#pragma unroll
+    for (int d = 0; d < 3; ++d) sv[d] = div_rn(mul_rn(R(2), t[d]), den);
+    const R v0 = add_rn(um[0], sub_rn(mul_rn(up[1], sv[2]), mul_rn(up[2], sv[1])));
+    const R v1 = add_rn(um[1], sub_rn(mul_rn(up[2], sv[0]), mul_rn(up[0], sv[2])));
+    const R v2 = add_rn(um[2], sub_rn(mul_rn(up[0], sv[1]), mul_rn(up[1], sv[0])));
+    u[0] = add_rn(v0, mul_rn(kq, E[0]));
+    u[1] = add_rn(v1, mul_rn(kq, E[1]));
+    u[2] = add_rn(v2, mul_rn(kq, E[2]));
+    return;
+  }
   R um0 = u[0] + kq * E[0], um1 = u[1] + kq * E[1], um2 = u[2] + kq * E[2];
   R ig = R(1) / sqrt(R(1) + (um0 * um0 + um1 * um1 + um2 * um2) * inv_c2);
   R t0 = kq * B[0] * ig, t1 = kq * B[1] * ig, t2 = kq * B[2] * ig;
@@ -75,6 +106,40 @@ __device__ __forceinline__ void boris(R kq, R inv_c2, const R* E, const R* B, R*
 // u_new = (u' + (u'.t) t + u' x t) / (1 + t^2)
 template <class R>
 __device__ __forceinline__ void vay(R kq, R inv_c2, const R* E, const R* B, R* u) {
+  if constexpr (kStatementOrder<R>) {
+    auto dot3 = [](const R* a, const R* b) {
+      return add_rn(add_rn(mul_rn(a[0], b[0]), mul_rn(a[1], b[1])), mul_rn(a[2], b[2]));
+    };
+    const R g0 = sqrt_rn(add_rn(R(1), mul_rn(dot3(u, u), inv_c2)));
+    const R v[3] = {div_rn(u[0], g0), div_rn(u[1], g0), div_rn(u[2], g0)};
+    R up[3], tau[3], t[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const int a = (d + 1) % 3, b = (d + 2) % 3;
+      up[d] = add_rn(add_rn(u[d], mul_rn(mul_rn(R(2), kq), E[d])),
+                     mul_rn(kq, sub_rn(mul_rn(v[a], B[b]), mul_rn(v[b], B[a]))));
+      tau[d] = mul_rn(kq, B[d]);
+    }
+    const R tau2 = dot3(tau, tau);
+    const R us = mul_rn(dot3(up, tau), sqrt_rn(inv_c2));
+    const R gp2 = add_rn(R(1), mul_rn(dot3(up, up), inv_c2));
+    const R sigma = sub_rn(gp2, tau2);
+    const R gn = sqrt_rn(div_rn(
+        add_rn(sigma, sqrt_rn(add_rn(mul_rn(sigma, sigma), mul_rn(R(4), add_rn(tau2, mul_rn(us, us)))))), R(2)));
+#pragma unroll
+    for (int d = 0; d < 3; ++d) t[d] = div_rn(tau[d], gn);
+    const R t2 = dot3(t, t);
+    const R ut = dot3(up, t);
+    const R sc = div_rn(R(1), add_rn(R(1), t2));
+    R un[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      const int a = (d + 1) % 3, b = (d + 2) % 3;
+      un[d] = mul_rn(sc, add_rn(add_rn(up[d], mul_rn(ut, t[d])), sub_rn(mul_rn(up[a], t[b]), mul_rn(up[b], t[a]))));
+    }
+    u[0] = un[0]; u[1] = un[1]; u[2] = un[2];
+    return;
+  }
   const R ig0 = R(1) / sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * inv_c2);
   const R v0 = u[0] * ig0, v1 = u[1] * ig0, v2 = u[2] * ig0;
   const R up0 = u[0] + R(2) * kq * E[0] + kq * (v1 * B[2] - v2 * B[1]);
@@ -101,6 +166,20 @@ __device__ __forceinline__ void push_momentum(int pusher, R kq, R inv_c2, const 
   else boris<R>(kq, inv_c2, E, B, u);
 }
 
+// step 2d: x~ = x + dt u / gamma(u), unwrapped
+template <class R>
+__device__ __forceinline__ void advance(R dt, R inv_c2, const R* x0, const R* u, R* x1) {
+  if constexpr (kStatementOrder<R>) {
+    const R g = sqrt_rn(add_rn(R(1), mul_rn(add_rn(add_rn(mul_rn(u[0], u[0]), mul_rn(u[1], u[1])), mul_rn(u[2], u[2])), inv_c2)));
+#pragma unroll
+    for (int d = 0; d < 3; ++d) x1[d] = add_rn(x0[d], div_rn(mul_rn(dt, u[d]), g));
+  } else {
+    const R ig = dt / sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * inv_c2);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) x1[d] = x0[d] + u[d] * ig;
+  }
+}
+
 // ------------------------------------------------------------------ Esirkepov, per axis set-up
 // Old and new nodal weights on a COMPACT window of ORDER+2 nodes that starts at grid index
 // `base` = min(l0, l1): the (ORDER+3)-wide window of the definition minus the slot that holds
@@ -121,7 +200,7 @@ __device__ __forceinline__ int esirkepov_axis(R xi0, R xi1, R* S0, R* DS) {
     R b_lo = i <= ORDER ? w1[i <= ORDER ? i : 0] : R(0);
     R b_hi = i >= 1 ? w1[i >= 1 ? i - 1 : 0] : R(0);
     S0[i] = o0 ? a_hi : a_lo;
-    DS[i] = (o1 ? b_hi : b_lo) - S0[i];
+    DS[i] = sub_rn(o1 ? b_hi : b_lo, S0[i]);
   }
   return o0 ? l1 : l0;
 }
@@ -134,7 +213,7 @@ __device__ __forceinline__ void deposit_global(const Grid<R>& g, const R* jf, R 
   int b[3];
 #pragma unroll
   for (int d = 0; d < 3; ++d) {
-    b[d] = esirkepov_axis<R, ORDER>(x0[d] * g.inv_dx[d], x1[d] * g.inv_dx[d], S0[d], DS[d]);
+    b[d] = esirkepov_axis<R, ORDER>(mul_rn(x0[d], g.inv_dx[d]), mul_rn(x1[d], g.inv_dx[d]), S0[d], DS[d]);
     b[d] = min(max(b[d], -kGuard), g.N[d] + kGuard - NW);
   }
   const int base = g.idx(b[0], b[1], b[2]);

@@ -27,8 +27,8 @@ __global__ void __launch_bounds__(128) k_particles_global(Grid<R> g, Particles<R
   R E[3], B[3];
   gather6<R, ORDER>(g, x0[0], x0[1], x0[2], E, B);
   push_momentum<R>(g.pusher, p.kq, g.inv_c2, E, B, u);
-  R ig = g.dt / sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * g.inv_c2);
-  R x1[3] = {x0[0] + u[0] * ig, x0[1] + u[1] * ig, x0[2] + u[2] * ig};
+  R x1[3];
+  advance<R>(g.dt, g.inv_c2, x0, u, x1);
   deposit_global<R, ORDER>(g, p.jf, w, x0, x1);
   bool out = false;
 #pragma unroll
@@ -53,10 +53,9 @@ __global__ void __launch_bounds__(128) k_push(Grid<R> g, Particles<R> p, R* __re
   R E[3], B[3];
   gather6<R, ORDER>(g, x0[0], x0[1], x0[2], E, B);
   push_momentum<R>(g.pusher, p.kq, g.inv_c2, E, B, u);
-  R ig = g.dt / sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * g.inv_c2);
-  xn[t] = x0[0] + u[0] * ig;
-  yn[t] = x0[1] + u[1] * ig;
-  zn[t] = x0[2] + u[2] * ig;
+  R x1[3];
+  advance<R>(g.dt, g.inv_c2, x0, u, x1);
+  xn[t] = x1[0]; yn[t] = x1[1]; zn[t] = x1[2];
   p.ux[t] = u[0]; p.uy[t] = u[1]; p.uz[t] = u[2];
 }
 
@@ -98,7 +97,7 @@ __device__ __forceinline__ void axis_record(R xi0, R xi1, int N, int& cell, R* S
     }
     S0[i] = a;
     S1[i] = b;
-    DS[i] = b - a;
+    DS[i] = sub_rn(b, a);
   }
   edge = (S0[0] != R(0)) | (S1[0] != R(0)) | (S0[NW - 1] != R(0)) | (S1[NW - 1] != R(0));
   cell = c;
@@ -182,7 +181,7 @@ __global__ void __launch_bounds__(kCoopWarps * 32) k_deposit_coop(Grid<R> g, Par
       bool edge[3];
 #pragma unroll
       for (int d = 0; d < 3; ++d)
-        axis_record<R, ORDER>(x0[d] * g.inv_dx[d], x1[d] * g.inv_dx[d], g.N[d], c[d], S0[d], DS[d], edge[d]);
+        axis_record<R, ORDER>(mul_rn(x0[d], g.inv_dx[d]), mul_rn(x1[d], g.inv_dx[d]), g.N[d], c[d], S0[d], DS[d], edge[d]);
       elig = cell_sorted == nullptr || cell_sorted[t] == c[0] + g.N[0] * (c[1] + g.N[1] * c[2]);
       if (NW * NW > 32) elig &= !(edge[1] && edge[2]);
       if (elig) {
@@ -308,7 +307,7 @@ __global__ void __launch_bounds__(128) k_deposit_list_warp(Grid<R> g, Particles<
       const R* a0 = lane == 0 ? p.x : (lane == 1 ? p.y : p.z);
       const R* a1 = lane == 0 ? xn : (lane == 1 ? yn : zn);
       R S0[NW], DS[NW];
-      int b = esirkepov_axis<R, ORDER>(a0[t] * g.inv_dx[lane], a1[t] * g.inv_dx[lane], S0, DS);
+      int b = esirkepov_axis<R, ORDER>(mul_rn(a0[t], g.inv_dx[lane]), mul_rn(a1[t], g.inv_dx[lane]), S0, DS);
       b = min(max(b, -kGuard), g.N[lane] + kGuard - NW);
       s_b[warp][lane] = b;
       R pre = 0;

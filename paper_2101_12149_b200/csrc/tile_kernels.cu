@@ -68,6 +68,16 @@ template <class R, int ORDER, int NX = ORDER + 1, int NY = ORDER + 1, int NZ = O
 __device__ __forceinline__ R interp_box(const R* __restrict__ F, int base, const R* wx, const R* wy, const R* wz) {
   constexpr int E = PushBox<ORDER>::EXT, SX = PushBox<ORDER>::SX;
   R acc = 0;
+  if constexpr (kStatementOrder<R>) {   // sum over c, b, a (a innermost) of ((wx wy) wz) F, every operation rounded
+#pragma unroll
+    for (int c = 0; c < NZ; ++c)
+#pragma unroll
+      for (int b = 0; b < NY; ++b)
+#pragma unroll
+        for (int a = 0; a < NX; ++a)
+          acc = add_rn(acc, mul_rn(mul_rn(mul_rn(wx[a], wy[b]), wz[c]), F[base + SX * a + b + E * c]));
+    return acc;
+  }
 #pragma unroll
   for (int c = 0; c < NZ; ++c) {
     R accb = 0;
@@ -88,10 +98,9 @@ __device__ __forceinline__ void push_store(const Grid<R>& g, const Particles<R>&
                                            R* __restrict__ yn, R* __restrict__ zn, int t, const R* x0, R* u,
                                            const R* Ef, const R* Bf) {
   push_momentum<R>(PUSHER, p.kq, g.inv_c2, Ef, Bf, u);   // compile-time constant: the other branch folds away
-  R ig = g.dt / sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * g.inv_c2);
-  xn[t] = x0[0] + u[0] * ig;
-  yn[t] = x0[1] + u[1] * ig;
-  zn[t] = x0[2] + u[2] * ig;
+  R x1[3];
+  advance<R>(g.dt, g.inv_c2, x0, u, x1);
+  xn[t] = x1[0]; yn[t] = x1[1]; zn[t] = x1[2];
   p.ux[t] = u[0]; p.uy[t] = u[1]; p.uz[t] = u[2];
 }
 
@@ -149,10 +158,10 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
     bool inbox = true;
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
-      R xi = x0[d] * g.inv_dx[d];
+      const R xi = mul_rn(x0[d], g.inv_dx[d]);
+      const R xs = sub_rn(xi, R(0.5));
       ln[d] = shape<R, ORDER>(xi, wn[d]) - (d == 0 ? o0 : (d == 1 ? o1 : o2));
-      ls[d] = (GATHER == 1 ? shape_lowered<R, ORDER>(xi - R(0.5), ws[d])
-                                         : shape<R, ORDER>(xi - R(0.5), ws[d])) -
+      ls[d] = (GATHER == 1 ? shape_lowered<R, ORDER>(xs, ws[d]) : shape<R, ORDER>(xs, ws[d])) -
               (d == 0 ? o0 : (d == 1 ? o1 : o2));
       inbox &= (ln[d] >= 0) & (ln[d] <= E - ORDER - 1) & (ls[d] >= 0) & (ls[d] <= E - ORDER - 1);
     }
@@ -252,7 +261,7 @@ __device__ __forceinline__ void axis_window(R xi0, R xi1, int& cell, R* S0, R* D
       b = (i == sl1 + k) ? w1[k] : b;
     }
     S0[i] = a;
-    DS[i] = b - a;
+    DS[i] = sub_rn(b, a);
   }
   fits = (so0 >= 0) & (so0 + ORDER < NW) & (sl1 >= 0) & (sl1 + ORDER < NW);
 }
@@ -408,9 +417,9 @@ __global__ void __launch_bounds__(NWARP * 32, 2)
       R S0x[NX], DSx[NX], S0y[NYZ], DSy[NYZ], S0z[NYZ], DSz[NYZ];
       int c[3];
       bool fit[3];
-      axis_window<R, ORDER, NX, W::BLX>(x0[0] * g.inv_dx[0], x1[0] * g.inv_dx[0], c[0], S0x, DSx, fit[0]);
-      axis_window<R, ORDER, NYZ, W::BLYZ>(x0[1] * g.inv_dx[1], x1[1] * g.inv_dx[1], c[1], S0y, DSy, fit[1]);
-      axis_window<R, ORDER, NYZ, W::BLYZ>(x0[2] * g.inv_dx[2], x1[2] * g.inv_dx[2], c[2], S0z, DSz, fit[2]);
+      axis_window<R, ORDER, NX, W::BLX>(mul_rn(x0[0], g.inv_dx[0]), mul_rn(x1[0], g.inv_dx[0]), c[0], S0x, DSx, fit[0]);
+      axis_window<R, ORDER, NYZ, W::BLYZ>(mul_rn(x0[1], g.inv_dx[1]), mul_rn(x1[1], g.inv_dx[1]), c[1], S0y, DSy, fit[1]);
+      axis_window<R, ORDER, NYZ, W::BLYZ>(mul_rn(x0[2], g.inv_dx[2]), mul_rn(x1[2], g.inv_dx[2]), c[2], S0z, DSz, fit[2]);
       const int rc0 = c[0] - tb[0], rc1 = c[1] - tb[1], rc2 = c[2] - tb[2];
       elig = fit[0] & fit[1] & fit[2] & (rc0 >= 0) & (rc0 < ts.T[0]) & (rc1 >= 0) & (rc1 < ts.T[1]) & (rc2 >= 0) &
              (rc2 < ts.T[2]);
@@ -621,9 +630,9 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
       R S0x[NX], DSx[NX], S0y[NYZ], DSy[NYZ], S0z[NYZ], DSz[NYZ];
       int c[3];
       bool fit[3];
-      axis_window<R, ORDER, NX, BLX>(x0[0] * g.inv_dx[0], x1[0] * g.inv_dx[0], c[0], S0x, DSx, fit[0]);
-      axis_window<R, ORDER, NYZ, BLYZ>(x0[1] * g.inv_dx[1], x1[1] * g.inv_dx[1], c[1], S0y, DSy, fit[1]);
-      axis_window<R, ORDER, NYZ, BLYZ>(x0[2] * g.inv_dx[2], x1[2] * g.inv_dx[2], c[2], S0z, DSz, fit[2]);
+      axis_window<R, ORDER, NX, BLX>(mul_rn(x0[0], g.inv_dx[0]), mul_rn(x1[0], g.inv_dx[0]), c[0], S0x, DSx, fit[0]);
+      axis_window<R, ORDER, NYZ, BLYZ>(mul_rn(x0[1], g.inv_dx[1]), mul_rn(x1[1], g.inv_dx[1]), c[1], S0y, DSy, fit[1]);
+      axis_window<R, ORDER, NYZ, BLYZ>(mul_rn(x0[2], g.inv_dx[2]), mul_rn(x1[2], g.inv_dx[2]), c[2], S0z, DSz, fit[2]);
       // the cell must be inside the grid and within 4 cells of the tile (4-bit biased offsets)
       const int rc0 = c[0] - tb[0] + 4, rc1 = c[1] - tb[1] + 4, rc2 = c[2] - tb[2] + 4;
       elig = fit[0] & fit[1] & fit[2] & (((rc0 | rc1 | rc2) & ~15) == 0) & (c[0] >= 0) & (c[0] < g.N[0]) &

@@ -1,0 +1,230 @@
+"""BASELINE.json configs 4 and 5 at their CONFIGURED size (north_star: "on all five configs"), in the launch
+configuration bench.py uses for them. The oracle cannot run 29 M / 134 M particles in test time, so, as for
+C2 and C3 (test_gpu_parity.test_full_size_sampled_parity_and_invariants):
+ (1) sort: every particle's cell index against the S-rule evaluated in numpy, keys non-decreasing, ties in
+     ascending old index, ids carried — the properties that define the unique stable sort (24-bit keys,
+     16.8 M bins);
+ (2) sampled sub-boxes: every particle near a box is pushed and deposited by the oracle one by one from the
+     GPU's state, and x, u, w of those particles, J on the inner nodes of the box and — where J is complete —
+     the E and B of the next step must match the GPU to the one-step tolerance;
+ (3) invariants that hold at any size: total charge exact, Gauss residual constant, nothing deactivated.
+C4 is the mesh-heavy 2-ppc laser-wakefield shape with the truncated z axis; C5 is the hot
+two-species disorder stress, taken through its re-sort at step 4 with the per-particle (stray)
+pass really hit."""
+import numpy as np
+import pytest
+
+import workloads as W
+from helpers import family_err, make_pair
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-12
+
+
+def _cells(p, cfg):
+    return [np.floor(p[k] / cfg.dx[a]).astype(np.int32) for a, k in enumerate("xyz")]
+
+
+def _check_sort(cfg, cell, perm, x_pre):
+    """(1): `cell`, `perm` of the most recent sort against positions `x_pre` (order before that sort)."""
+    n = cfg.n_cells
+    npart = len(perm)
+    assert np.array_equal(np.sort(perm), np.arange(npart, dtype=perm.dtype))
+    want = np.zeros(npart, dtype=np.int64)
+    for a in (2, 1, 0):       # S-rule: one rounded multiply, floor, clamp; cell = cx + Nx (cy + Ny cz)
+        ca = np.clip(np.floor(x_pre[a][perm] * cfg.np_dtype(1.0 / cfg.dx[a])).astype(np.int64), 0, n[a] - 1)
+        want = want * n[a] + ca
+    assert np.array_equal(cell.astype(np.int64), want)
+    del want
+    T = cfg.tile
+    cell = cell.astype(np.int64)
+    ci, cj, ck = cell % n[0], (cell // n[0]) % n[1], cell // (n[0] * n[1])
+    nt = (n[0] // T[0], n[1] // T[1], n[2] // T[2])
+    key = ((ci // T[0]) + nt[0] * ((cj // T[1]) + nt[1] * (ck // T[2]))) * (T[0] * T[1] * T[2]) + \
+        (ci % T[0]) + T[0] * ((cj % T[1]) + T[1] * (ck % T[2]))
+    dk = np.diff(key)
+    assert np.all(dk >= 0)
+    assert np.all(np.diff(perm.astype(np.int64))[dk == 0] > 0)          # stable: ties keep ascending old index
+
+
+def _near(cc, cfg, lo, size, margin):
+    """particles whose cell lies within `margin` cells of the box [lo, lo+size) (modulo N on periodic axes)"""
+    sel = np.ones(len(cc[0]), dtype=bool)
+    for a in range(3):
+        rel = cc[a] - (lo[a] - margin)
+        if cfg.periodic[a]:
+            rel = rel % cfg.n_cells[a]
+        sel &= (rel >= 0) & (rel < size[a] + 2 * margin)
+    return sel
+
+
+def _box_nodes(cfg, lo, size, shrink=0):
+    """np.ix_ index of the nodes [lo+shrink, lo+size-shrink) in (z, y, x) array order, wrapped / clipped"""
+    ax = []
+    for a in range(3):
+        i = np.arange(lo[a] + shrink, lo[a] + size[a] - shrink)
+        i = i % cfg.n_cells[a] if cfg.periodic[a] else i[(i >= 0) & (i < cfg.n_cells[a])]
+        ax.append(i)
+    return np.ix_(ax[2], ax[1], ax[0])
+
+
+def _oracle_for(cfg, E, B, sort_interval=0):
+    import oracle
+    o = oracle.Oracle(cfg.n_cells, cfg.dx, cfg.dt, cfg.order, dtype=cfg.np_dtype, periodic=cfg.periodic,
+                      sort_interval=sort_interval)
+    o.set_fields(E, B)
+    return o
+
+
+def test_C4_full_size_sampled_parity_and_invariants():
+    cfg = W.CONFIGS["C4"]
+    _, g, species = make_pair(cfg, with_oracle=False)
+    x_in = [species[0][1][k] for k in "xyz"]
+    spec = cfg.species[0]
+    del species
+    n = cfg.n_cells
+    d0 = g.diagnostics()
+    g.step(1)
+    cell, perm = g.get_sort_state(0)
+    _check_sort(cfg, cell, perm, x_in)                                  # (1) the sort of step 0
+    del x_in, cell
+    p = g.get_particles(0)
+    assert np.array_equal(p["id"], perm.astype(np.int64))
+    del p, perm
+    # after 101 steps the laser (loaded in z-cells 16..112, moving 0.93 cell per step) fills the density ramp
+    # (z-cells 128..192) and the electrons there are relativistic; step 101 does not sort
+    g.step(100)
+    p1 = g.get_particles(0)
+    E1, B1, _ = g.get_fields(with_J=False)
+    assert max(np.max(np.abs(p1[k])) for k in ("ux", "uy", "uz")) > 0.3 * W.C_LIGHT
+    cc = _cells(p1, cfg)
+    zfront = int(cc[2].min()) - 3                     # no particle, hence no J, in the planes below this one
+    assert zfront > 60
+    # (2) sub-boxes: in the ramp under the laser axis; across the end of the ramp, off axis; on the high z
+    # face in the periodic x-y corner (wraps in x and y, truncated in z)
+    boxes = [((58, 58, 150), (12, 12, 12)), ((30, 80, 186), (12, 12, 12)), ((-6, -6, 1012), (12, 12, 12))]
+    margin = 3
+    sel = np.zeros(len(cc[0]), dtype=bool)
+    for lo, size in boxes:
+        sel |= _near(cc, cfg, lo, size, margin)
+    idx = np.nonzero(sel)[0]
+    del cc, sel
+    assert 10000 < len(idx) < 400000
+    o = _oracle_for(cfg, E1, B1)
+    o.add_species(*[p1[k][idx] for k in ("x", "y", "z", "ux", "uy", "uz", "w")], spec.charge, spec.mass)
+    o.step(1)
+    g.step(1)
+    p2 = g.get_particles(0)
+    assert np.array_equal(p2["id"], p1["id"])
+    po = o.get_particles(0)
+    assert family_err([p2[k][idx] for k in "xyz"], [po[k] for k in "xyz"]) <= TOL64
+    assert family_err([p2[k][idx] for k in ("ux", "uy", "uz")], [po[k] for k in ("ux", "uy", "uz")]) <= TOL64
+    assert np.array_equal(p2["w"][idx], po["w"])
+    del p1, p2
+    Eg, Bg, Jg = g.get_fields()
+    Eo, Bo, Jo = o.get_fields()
+    jscale = max(np.max(np.abs(J)) for J in Jg)
+    escale = max(np.max(np.abs(F)) for F in Eg)
+    bscale = max(np.max(np.abs(F)) for F in Bg)
+    assert jscale > 0
+    for bi, (lo, size) in enumerate(boxes):
+        ix = _box_nodes(cfg, lo, size)
+        ix1 = _box_nodes(cfg, lo, size, shrink=1)       # the second B half step reads the new E one node up
+        for c in range(3):
+            assert np.max(np.abs(Jg[c][ix] - Jo[c][ix])) <= TOL64 * jscale
+            assert np.max(np.abs(Eg[c][ix] - Eo[c][ix])) <= TOL64 * escale
+            assert np.max(np.abs(Bg[c][ix1] - Bo[c][ix1])) <= TOL64 * bscale
+        if bi < 2:
+            assert max(np.max(np.abs(Jo[c][ix])) for c in range(3)) > 1e-3 * jscale   # the laser drives J here
+    # in front of the plasma J is zero on both sides: the tail of the laser, what the plasma sent back and the
+    # truncated low-z face evolve by the field solver alone and must match on every node
+    assert all(np.all(Jg[c][:zfront] == 0) for c in range(3))
+    for c in range(3):
+        assert np.max(np.abs(Eg[c][:zfront] - Eo[c][:zfront])) <= TOL64 * escale
+        assert np.max(np.abs(Bg[c][:zfront - 1] - Bo[c][:zfront - 1])) <= TOL64 * bscale
+    assert np.max(np.abs(Eg[0][:zfront])) > 1e-3 * escale
+    del Eg, Bg, Jg, Eo, Bo, Jo, o
+    # (3) invariants
+    g.step(6)                                                           # through the re-sort at step 104
+    d = g.diagnostics()
+    assert d["charge"] == pytest.approx(d0["charge"], rel=1e-12)
+    assert abs(d["gauss_max"] - d0["gauss_max"]) < 1e-9 * max(d0["rho_max"], d0["gauss_max"])
+    assert d["deactivated"] == 0
+
+
+def test_C5_full_size_two_species_through_the_resort():
+    cfg = W.CONFIGS["C5"]
+    _, g, species = make_pair(cfg, with_oracle=False)
+    x_in = [[arrs[k] for k in "xyz"] for _, arrs in species]
+    del species
+    nsp = len(cfg.species)
+    d0 = g.diagnostics()
+    g.step(1)
+    for s in range(nsp):                                                # (1) the sort of step 0, both species
+        cell, perm = g.get_sort_state(s)
+        _check_sort(cfg, cell, perm, x_in[s])
+        x_in[s] = None
+        del cell, perm
+    g.step(3)
+    # state after 4 steps; step 4 re-sorts (hot electrons: the order is stale) and then pushes
+    lo, size, margin = (100, 120, 60), (12, 12, 12), 3
+    E1, B1, _ = g.get_fields(with_J=False)
+    o = _oracle_for(cfg, E1, B1)
+    del E1, B1
+    pre = []
+    for s in range(nsp):
+        p1 = g.get_particles(s)
+        idx = np.nonzero(_near(_cells(p1, cfg), cfg, lo, size, margin))[0]
+        assert 5000 < len(idx) < 200000
+        spec = cfg.species[s]
+        o.add_species(*[p1[k][idx] for k in ("x", "y", "z", "ux", "uy", "uz", "w")], spec.charge, spec.mass)
+        pre.append(dict(sub_ids=p1["id"][idx], ids=p1["id"], x=[p1[k] for k in "xyz"],
+                        cyz=[np.floor(p1[k] / cfg.dx[a]).astype(np.int32) for a, k in ((1, "y"), (2, "z"))]))
+        del p1
+    o.step(1)
+    g.step(1)                                                           # step 4: sort, push, deposit
+    crossed = []
+    for s in range(nsp):
+        q = pre[s]
+        cell, perm = g.get_sort_state(s)
+        _check_sort(cfg, cell, perm, q["x"])                            # (1) again, on the drifted positions
+        del cell
+        p2 = g.get_particles(s)
+        assert np.array_equal(p2["id"], q["ids"][perm])                 # ids are carried through the sort
+        # how many left their cell in y or z during step 4 (these take the per-particle pass)
+        cyz2 = [np.floor(p2[k] / cfg.dx[a]).astype(np.int32) for a, k in ((1, "y"), (2, "z"))]
+        crossed.append(float(np.mean((cyz2[0] != q["cyz"][0][perm]) | (cyz2[1] != q["cyz"][1][perm]))))
+        del cyz2, perm
+        # (2) the sampled particles, matched by id
+        where = np.empty(len(p2["id"]), dtype=np.int64)
+        where[p2["id"]] = np.arange(len(p2["id"]))
+        at = where[q["sub_ids"]]
+        del where
+        po = o.get_particles(s)
+        assert family_err([p2[k][at] for k in "xyz"], [po[k] for k in "xyz"]) <= TOL64
+        assert family_err([p2[k][at] for k in ("ux", "uy", "uz")], [po[k] for k in ("ux", "uy", "uz")]) <= TOL64
+        assert np.array_equal(p2["w"][at], po["w"])
+        del p2
+        pre[s] = None
+    assert crossed[0] > 0.05, crossed                                    # hot electrons: the stray pass is really hit
+    assert crossed[1] < 0.01, crossed
+    Eg, Bg, Jg = g.get_fields()
+    Eo, Bo, Jo = o.get_fields()
+    jscale = max(np.max(np.abs(J)) for J in Jg)
+    escale = max(np.max(np.abs(F)) for F in Eg)
+    bscale = max(np.max(np.abs(F)) for F in Bg)
+    ix, ix1 = _box_nodes(cfg, lo, size), _box_nodes(cfg, lo, size, shrink=1)
+    for c in range(3):
+        assert np.max(np.abs(Jg[c][ix] - Jo[c][ix])) <= TOL64 * jscale
+        assert np.max(np.abs(Eg[c][ix] - Eo[c][ix])) <= TOL64 * escale
+        assert np.max(np.abs(Bg[c][ix1] - Bo[c][ix1])) <= TOL64 * bscale
+    assert max(np.max(np.abs(Jo[c][ix])) for c in range(3)) > 0.05 * jscale
+    del Eg, Bg, Jg, Eo, Bo, Jo, o
+    # (3) invariants
+    g.step(4)                                                           # through the re-sort at step 8
+    d = g.diagnostics()
+    qtot = W.Q_E * 1e25 * 1e-18 * 256 ** 3                              # charge of one species; the two cancel
+    assert abs(d["charge"] - d0["charge"]) < 1e-12 * qtot
+    assert abs(d["gauss_max"] - d0["gauss_max"]) < 1e-9 * d0["rho_max"]
+    assert d["deactivated"] == 0
