@@ -21,11 +21,11 @@ DIAG = ("field_E", "field_B", "kinetic", "charge", "gauss_max", "rho_max", "deac
 
 
 def build(force: bool = False) -> str:
-    """Compile the oracle (g++ -O2 -ffp-contract=off). Returns the library path."""
+    """Compile the oracle (g++ -O2 -ffp-contract=off -fopenmp). Returns the library path."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + ".tmp%d" % os.getpid()
         subprocess.check_call(
-            ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC",
+            ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC",
              "-o", tmp, _SRC])
         os.replace(tmp, _LIB)
     return _LIB
@@ -45,6 +45,8 @@ def lib():
         L.orc_add_species.argtypes = [vp, C.c_int64] + [vp] * 7 + [C.c_double, C.c_double]
         L.orc_set_fields.argtypes = [vp, C.POINTER(vp), C.POINTER(vp)]
         L.orc_step.argtypes = [vp, C.c_int]
+        L.orc_step_omp.argtypes = [vp, C.c_int, C.c_int]
+        L.orc_step_omp.restype = C.c_int
         L.orc_get_fields.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
         L.orc_num_particles.restype = C.c_int64
         L.orc_num_particles.argtypes = [vp, C.c_int]
@@ -174,6 +176,12 @@ class Oracle:
 
     def step(self, n=1):
         lib().orc_step(self._h, int(n))
+
+    def step_omp(self, n=1, threads=0) -> int:
+        """The OpenMP variant (the paper's CPU scheme: tiles to threads, private J buffers, one atomic per cell;
+        PAPER.md:171-173). Same arithmetic per particle as step(); J sums in another order. Returns the thread
+        count used (threads <= 0: all that OpenMP offers)."""
+        return lib().orc_step_omp(self._h, int(n), int(threads))
 
     def sort_now(self):
         lib().orc_sort_now(self._h)

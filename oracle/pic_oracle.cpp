@@ -19,11 +19,14 @@
 // unity and first moment (T1), Boris gyration angle/radius (T2), hyperbolic
 // motion (T3), Yee numerical dispersion (T4), Esirkepov continuity (T5), first
 // moment of J (T6), brute-force dense deposit (T7), Gauss-law constancy (T8),
-// plasma oscillation (T9), stable sort vs numpy (T10), order independence (T11).
-// Nothing here is "parity unpinned".
+// plasma oscillation (T9), stable sort vs numpy (T10), order independence (T11), the OpenMP variant against
+// the serial oracle (T12), Vay (T13), Galerkin gather (T14), CKC (T15), step 2f / diagnostics / truncated-axis
+// field reads (tests/test_oracle_pins_boundaries.py). Nothing here is "parity unpinned".
 //
-// Build: g++ -O2 -ffp-contract=off -shared -fPIC (no FMA contraction, so the
+// Build: g++ -O2 -ffp-contract=off -fopenmp -shared -fPIC (no FMA contraction, so the
 // integer cell rule below is one rounded multiply exactly as written).
+
+#include <omp.h>
 
 #include <cmath>
 #include <cstdint>
@@ -108,6 +111,7 @@ struct Sim {
   std::vector<Species<R>> sp;
   int64_t step_count = 0;
   int64_t n_deactivated = 0;
+  int omp_threads = 1;   // > 1 only inside the OpenMP variant (orc_step_omp)
 
   size_t ncell() const { return (size_t)N[0] * N[1] * N[2]; }
 
@@ -210,8 +214,8 @@ void vay(R kq, R inv_c2, const R E[3], const R B[3], R u[3]) {
 // Esirkepov charge-conserving deposit of one particle moving x0 -> x1
 // (x1 unwrapped), nodal shapes of order n, (n+3)-wide window per axis with
 // base b = l0-1 (reading Q5). J accumulates in double (reading Q10).
-template <class R>
-void deposit(Sim<R>& s, const Species<R>& sp, const R x0[3], const R x1[3], R wq) {
+template <class R, class Sink>
+void deposit_to(const Sim<R>& s, const Species<R>& sp, const R x0[3], const R x1[3], R wq, Sink&& add) {
   const int n = s.order, W = n + 3;
   R S0[3][6], S1[3][6], DS[3][6];
   int b[3];
@@ -238,8 +242,7 @@ void deposit(Sim<R>& s, const Species<R>& sp, const R x0[3], const R x1[3], R wq
         R Wx = DS[0][i] * (S0[1][j] * S0[2][k] + half * DS[1][j] * S0[2][k] +
                            half * S0[1][j] * DS[2][k] + third * DS[1][j] * DS[2][k]);
         pre += Wx;
-        int64_t t = s.lin(b[0] + i, b[1] + j, b[2] + k);
-        if (t >= 0) s.Jd[0][(size_t)t] += (double)(-(wq * sp.jf[0]) * pre);
+        add(0, b[0] + i, b[1] + j, b[2] + k, (double)(-(wq * sp.jf[0]) * pre));
       }
     }
   // Jy: prefix along j
@@ -250,8 +253,7 @@ void deposit(Sim<R>& s, const Species<R>& sp, const R x0[3], const R x1[3], R wq
         R Wy = DS[1][j] * (S0[0][i] * S0[2][k] + half * DS[0][i] * S0[2][k] +
                            half * S0[0][i] * DS[2][k] + third * DS[0][i] * DS[2][k]);
         pre += Wy;
-        int64_t t = s.lin(b[0] + i, b[1] + j, b[2] + k);
-        if (t >= 0) s.Jd[1][(size_t)t] += (double)(-(wq * sp.jf[1]) * pre);
+        add(1, b[0] + i, b[1] + j, b[2] + k, (double)(-(wq * sp.jf[1]) * pre));
       }
     }
   // Jz: prefix along k
@@ -262,10 +264,18 @@ void deposit(Sim<R>& s, const Species<R>& sp, const R x0[3], const R x1[3], R wq
         R Wz = DS[2][k] * (S0[0][i] * S0[1][j] + half * DS[0][i] * S0[1][j] +
                            half * S0[0][i] * DS[1][j] + third * DS[0][i] * DS[1][j]);
         pre += Wz;
-        int64_t t = s.lin(b[0] + i, b[1] + j, b[2] + k);
-        if (t >= 0) s.Jd[2][(size_t)t] += (double)(-(wq * sp.jf[2]) * pre);
+        add(2, b[0] + i, b[1] + j, b[2] + k, (double)(-(wq * sp.jf[2]) * pre));
       }
     }
+}
+
+// the canonical (serial) sink: straight into the global J, index rule of reading Q6
+template <class R>
+void deposit(Sim<R>& s, const Species<R>& sp, const R x0[3], const R x1[3], R wq) {
+  deposit_to<R>(s, sp, x0, x1, wq, [&](int c, int i, int j, int k, double v) {
+    int64_t t = s.lin(i, j, k);
+    if (t >= 0) s.Jd[c][(size_t)t] += v;
+  });
 }
 
 // ---------------------------------------------------------------- S-rules
@@ -291,7 +301,8 @@ void sort_species(Sim<R>& s, Species<R>& sp) {
   std::vector<int64_t> key(np);
   sp.cell.assign(np, 0);
   sp.perm.assign(np, 0);
-  for (size_t p = 0; p < np; ++p) {
+#pragma omp parallel for num_threads(s.omp_threads) if (s.omp_threads > 1) schedule(static)
+  for (int64_t p = 0; p < (int64_t)np; ++p) {
     int c[3] = {cell_of(s, 0, sp.x[p]), cell_of(s, 1, sp.y[p]), cell_of(s, 2, sp.z[p])};
     sp.cell[p] = c[0] + s.N[0] * (c[1] + s.N[1] * c[2]);
     int64_t t = (c[0] / T[0]) + (int64_t)nt[0] * ((c[1] / T[1]) + (int64_t)nt[1] * (c[2] / T[2]));
@@ -305,7 +316,8 @@ void sort_species(Sim<R>& s, Species<R>& sp) {
   // gather all arrays and id through perm; `cell` is stored in the new order
   auto permute = [&](auto& v) {
     auto old = v;
-    for (size_t k = 0; k < np; ++k) v[k] = old[(size_t)sp.perm[k]];
+#pragma omp parallel for num_threads(s.omp_threads) if (s.omp_threads > 1) schedule(static)
+    for (int64_t k = 0; k < (int64_t)np; ++k) v[(size_t)k] = old[(size_t)sp.perm[(size_t)k]];
   };
   permute(sp.x); permute(sp.y); permute(sp.z);
   permute(sp.ux); permute(sp.uy); permute(sp.uz);
@@ -319,6 +331,7 @@ template <class R>
 void push_B_half(Sim<R>& s) {
   auto &Ex = s.F[0], &Ey = s.F[1], &Ez = s.F[2];
   std::vector<R> nBx(s.F[3]), nBy(s.F[4]), nBz(s.F[5]);
+#pragma omp parallel for num_threads(s.omp_threads) if (s.omp_threads > 1) schedule(static)
   for (int k = 0; k < s.N[2]; ++k)
     for (int j = 0; j < s.N[1]; ++j)
       for (int i = 0; i < s.N[0]; ++i) {
@@ -358,6 +371,7 @@ template <class R>
 void push_B_half_ckc(Sim<R>& s) {
   auto &Ex = s.F[0], &Ey = s.F[1], &Ez = s.F[2];
   std::vector<R> nBx(s.F[3]), nBy(s.F[4]), nBz(s.F[5]);
+#pragma omp parallel for num_threads(s.omp_threads) if (s.omp_threads > 1) schedule(static)
   for (int k = 0; k < s.N[2]; ++k)
     for (int j = 0; j < s.N[1]; ++j)
       for (int i = 0; i < s.N[0]; ++i) {
@@ -378,6 +392,7 @@ void push_B(Sim<R>& s) {
 template <class R>
 void push_E(Sim<R>& s) {
   auto &Bx = s.F[3], &By = s.F[4], &Bz = s.F[5];
+#pragma omp parallel for num_threads(s.omp_threads) if (s.omp_threads > 1) schedule(static)
   for (int k = 0; k < s.N[2]; ++k)
     for (int j = 0; j < s.N[1]; ++j)
       for (int i = 0; i < s.N[0]; ++i) {
@@ -390,48 +405,126 @@ void push_E(Sim<R>& s) {
 }
 
 // ---------------------------------------------------------------- one step
+// steps 2b-2g for particle p of one species; `add` receives the particle's J contributions (step 2e)
+template <class R, class Sink>
+inline void particle_one(const Sim<R>& s, Species<R>& sp, size_t p, Sink&& add, int64_t& n_deactivated) {
+  R x0[3] = {sp.x[p], sp.y[p], sp.z[p]};
+  R u[3] = {sp.ux[p], sp.uy[p], sp.uz[p]};
+  R E[3], B[3];
+  for (int c = 0; c < 3; ++c) {                        // 2b
+    E[c] = gather<R>(s, c, x0[0], x0[1], x0[2]);
+    B[c] = gather<R>(s, 3 + c, x0[0], x0[1], x0[2]);
+  }
+  if (s.pusher == 1) vay<R>(sp.kq, s.inv_c2, E, B, u);
+  else boris<R>(sp.kq, s.inv_c2, E, B, u);             // 2c
+  R g = std::sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * s.inv_c2);
+  R x1[3];
+  for (int d = 0; d < 3; ++d) x1[d] = x0[d] + s.dtr * u[d] / g;   // 2d (unwrapped)
+  R w = sp.w[p];
+  deposit_to<R>(s, sp, x0, x1, w, add);                // 2e
+  for (int d = 0; d < 3; ++d) {                        // 2f
+    if (s.periodic[d]) {
+      if (x1[d] < R(0)) x1[d] += s.L[d];
+      if (x1[d] >= s.L[d]) x1[d] -= s.L[d];
+    } else if (!(x1[d] >= R(0) && x1[d] < s.L[d])) {
+      if (w != R(0)) n_deactivated++;
+      w = R(0);
+      x1[d] = x1[d] < R(0) ? R(0) : std::nextafter(s.L[d], R(0));
+    }
+  }
+  sp.x[p] = x1[0]; sp.y[p] = x1[1]; sp.z[p] = x1[2];   // 2g
+  sp.ux[p] = u[0]; sp.uy[p] = u[1]; sp.uz[p] = u[2];
+  sp.w[p] = w;
+}
+
+// the canonical oracle: every particle in current array order, contributions summed straight into J
 template <class R>
 void particles_step(Sim<R>& s) {
+  auto into_J = [&](int c, int i, int j, int k, double v) {
+    int64_t t = s.lin(i, j, k);
+    if (t >= 0) s.Jd[c][(size_t)t] += v;
+  };
+  for (auto& sp : s.sp)
+    for (size_t p = 0; p < sp.x.size(); ++p) particle_one<R>(s, sp, p, into_J, s.n_deactivated);
+}
+
+// ---------------------------------------------------------------- OpenMP variant (pin T12)
+// The paper's CPU scheme: the particles are binned onto tiles, OpenMP threads take
+// tiles, each thread deposits its tile's particles onto a PRIVATE buffer with enough cells to capture the
+// support of every particle of the tile (no atomics), and then adds the buffer to the full grid with one
+// atomic per CELL instead of one per particle-node. The per-particle arithmetic is particle_one, unchanged;
+// only the order in which contributions reach J differs from the canonical oracle, so the two agree to
+// summation roundoff (T12: 1e-13 of max). Used for the N-core baseline of bench.py, never as the checker.
+template <class R>
+void particles_step_omp(Sim<R>& s, int nthreads) {
+  const int* T = s.tile;
+  const int nt[3] = {s.N[0] / T[0], s.N[1] / T[1], s.N[2] / T[2]};
+  const int64_t ntiles = (int64_t)nt[0] * nt[1] * nt[2];
+  // nodes a particle of cell c can touch: c-2 .. c+4 (order 2: l0 in {c-1, c}, window l0-1 .. l0+n+1)
+  const int lo = 2, ext[3] = {T[0] + 7, T[1] + 7, T[2] + 7};
+  const size_t bvol = (size_t)ext[0] * ext[1] * ext[2];
   for (auto& sp : s.sp) {
-    size_t np = sp.x.size();
-    for (size_t p = 0; p < np; ++p) {
-      R x0[3] = {sp.x[p], sp.y[p], sp.z[p]};
-      R u[3] = {sp.ux[p], sp.uy[p], sp.uz[p]};
-      R E[3], B[3];
-      for (int c = 0; c < 3; ++c) {                        // 2b
-        E[c] = gather<R>(s, c, x0[0], x0[1], x0[2]);
-        B[c] = gather<R>(s, 3 + c, x0[0], x0[1], x0[2]);
-      }
-      if (s.pusher == 1) vay<R>(sp.kq, s.inv_c2, E, B, u);
-      else boris<R>(sp.kq, s.inv_c2, E, B, u);             // 2c
-      R g = std::sqrt(R(1) + (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]) * s.inv_c2);
-      R x1[3];
-      for (int d = 0; d < 3; ++d) x1[d] = x0[d] + s.dtr * u[d] / g;   // 2d (unwrapped)
-      R w = sp.w[p];
-      deposit<R>(s, sp, x0, x1, w);                        // 2e
-      for (int d = 0; d < 3; ++d) {                        // 2f
-        if (s.periodic[d]) {
-          if (x1[d] < R(0)) x1[d] += s.L[d];
-          if (x1[d] >= s.L[d]) x1[d] -= s.L[d];
-        } else if (!(x1[d] >= R(0) && x1[d] < s.L[d])) {
-          if (w != R(0)) s.n_deactivated++;
-          w = R(0);
-          x1[d] = x1[d] < R(0) ? R(0) : std::nextafter(s.L[d], R(0));
-        }
-      }
-      sp.x[p] = x1[0]; sp.y[p] = x1[1]; sp.z[p] = x1[2];   // 2g
-      sp.ux[p] = u[0]; sp.uy[p] = u[1]; sp.uz[p] = u[2];
-      sp.w[p] = w;
+    const size_t np = sp.x.size();
+    // bin the particles onto tiles by their current cell (stable: ascending index inside a tile)
+    std::vector<int64_t> start((size_t)ntiles + 1, 0);
+    std::vector<int32_t> tile_of(np), list(np);
+#pragma omp parallel for num_threads(nthreads) schedule(static)
+    for (int64_t p = 0; p < (int64_t)np; ++p) {
+      int c[3] = {cell_of(s, 0, sp.x[p]), cell_of(s, 1, sp.y[p]), cell_of(s, 2, sp.z[p])};
+      tile_of[p] = (int32_t)((c[0] / T[0]) + (int64_t)nt[0] * ((c[1] / T[1]) + (int64_t)nt[1] * (c[2] / T[2])));
     }
+    for (size_t p = 0; p < np; ++p) start[(size_t)tile_of[p] + 1]++;
+    for (int64_t t = 0; t < ntiles; ++t) start[(size_t)t + 1] += start[(size_t)t];
+    {
+      std::vector<int64_t> fill(start.begin(), start.end() - 1);
+      for (size_t p = 0; p < np; ++p) list[(size_t)fill[(size_t)tile_of[p]]++] = (int32_t)p;
+    }
+    int64_t deact = 0;
+#pragma omp parallel num_threads(nthreads) reduction(+ : deact)
+    {
+      std::vector<double> buf[3];
+      for (int c = 0; c < 3; ++c) buf[c].assign(bvol, 0.0);
+#pragma omp for schedule(dynamic, 1)
+      for (int64_t t = 0; t < ntiles; ++t) {
+        if (start[(size_t)t] == start[(size_t)t + 1]) continue;
+        const int t0[3] = {(int)(t % nt[0]) * T[0] - lo, (int)((t / nt[0]) % nt[1]) * T[1] - lo,
+                           (int)(t / ((int64_t)nt[0] * nt[1])) * T[2] - lo};
+        auto into_buf = [&](int c, int i, int j, int k, double v) {
+          buf[c][(size_t)(i - t0[0]) + (size_t)ext[0] * ((size_t)(j - t0[1]) + (size_t)ext[1] * (size_t)(k - t0[2]))] += v;
+        };
+        for (int64_t q = start[(size_t)t]; q < start[(size_t)t + 1]; ++q)
+          particle_one<R>(s, sp, (size_t)list[(size_t)q], into_buf, deact);
+        // flush: one atomic per touched cell, index rule of reading Q6 (modulo / dropped)
+        for (int c = 0; c < 3; ++c)
+          for (int k = 0; k < ext[2]; ++k)
+            for (int j = 0; j < ext[1]; ++j)
+              for (int i = 0; i < ext[0]; ++i) {
+                double& v = buf[c][(size_t)i + (size_t)ext[0] * ((size_t)j + (size_t)ext[1] * (size_t)k)];
+                if (v == 0.0) continue;
+                int64_t g = s.lin(t0[0] + i, t0[1] + j, t0[2] + k);
+                if (g >= 0) {
+#pragma omp atomic
+                  s.Jd[c][(size_t)g] += v;
+                }
+                v = 0.0;
+              }
+      }
+    }
+    s.n_deactivated += deact;
   }
 }
 
+// nthreads = 1: the canonical serial oracle. nthreads > 1: the OpenMP variant (particles by tile with private
+// J buffers; the node loops of the field solver and the gathers of the sort split over threads — every
+// node / slot is independent, so those are bit-identical to the serial loops).
 template <class R>
-void step(Sim<R>& s) {
+void step(Sim<R>& s, int nthreads = 1) {
+  s.omp_threads = nthreads;
   if (s.sort_interval > 0 && s.step_count % s.sort_interval == 0)   // 0
     for (auto& sp : s.sp) sort_species<R>(s, sp);
   for (int c = 0; c < 3; ++c) std::fill(s.Jd[c].begin(), s.Jd[c].end(), 0.0);  // 1
-  particles_step<R>(s);                                             // 2
+  if (nthreads > 1) particles_step_omp<R>(s, nthreads);
+  else particles_step<R>(s);                                        // 2
   for (int c = 0; c < 3; ++c)
     for (size_t t = 0; t < s.ncell(); ++t) s.J[c][t] = (R)s.Jd[c][t];
   push_B<R>(s);                                                     // 3
@@ -641,6 +734,18 @@ void orc_step(void* hv, int n) {
   for (int i = 0; i < n; ++i) {
     if (h->prec == 0) step<double>(*h->d); else step<float>(*h->f);
   }
+}
+
+// OpenMP variant of orc_step (pin T12); nthreads <= 0: all the threads OpenMP offers.
+// Returns the thread count used.
+int orc_step_omp(void* hv, int n, int nthreads) {
+  auto* h = (Handle*)hv;
+  if (nthreads <= 0) nthreads = omp_get_max_threads();
+  for (int i = 0; i < n; ++i) {
+    if (h->prec == 0) step<double>(*h->d, nthreads); else step<float>(*h->f, nthreads);
+  }
+  if (h->prec == 0) h->d->omp_threads = 1; else h->f->omp_threads = 1;
+  return nthreads;
 }
 
 void orc_get_fields(void* hv, void* const* E, void* const* B, void* const* J) {

@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_HERE, "libpic.so")
 PIC_F64, PIC_F32 = 0, 1
 PIC_HOST, PIC_DEVICE = 0, 1
 PIC_DEPOSIT_AUTO, PIC_DEPOSIT_GLOBAL, PIC_DEPOSIT_COOP, PIC_DEPOSIT_TILE, PIC_DEPOSIT_TILE_MMA = 0, 1, 2, 3, 4
+PIC_DEPOSIT_FUSED = 5
 PIC_PUSHER_BORIS, PIC_PUSHER_VAY = 0, 1
 PIC_GATHER_UNIFORM, PIC_GATHER_GALERKIN = 0, 1
 PIC_SOLVER_YEE, PIC_SOLVER_CKC = 0, 1

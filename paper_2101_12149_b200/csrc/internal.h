@@ -1,5 +1,6 @@
 // Host-side declarations shared by the translation units of libpic.so (CUDA path only).
 #pragma once
+#include <set>
 #include <vector>
 
 #include "common.cuh"
@@ -48,6 +49,21 @@ struct Timer {
     }
     spans.clear();
   }
+  void fold_completed() {   // folds the leading spans whose end event has already completed; never waits
+    size_t k = 0;
+    for (; k < spans.size(); ++k) {
+      auto& s = spans[k];
+      if (cudaEventQuery(s.b) != cudaSuccess) break;
+      float t = 0;
+      cudaEventElapsedTime(&t, s.a, s.b);
+      ms[s.phase] += t;
+      count[s.phase] += 1;
+      free_events.push_back(s.a);
+      free_events.push_back(s.b);
+    }
+    cudaGetLastError();   // cudaErrorNotReady is not an error here
+    spans.erase(spans.begin(), spans.begin() + k);
+  }
   void reset() {
     for (int i = 0; i < kNumPhases; ++i) { ms[i] = 0; count[i] = 0; }
   }
@@ -61,6 +77,9 @@ struct Timer {
 
 struct Ctx {
   cudaStream_t stream = nullptr;
+  int device = 0;         // the device the handle was created on
+  int sm_count = 148;     // its multiProcessorCount (grid sizing of the grid-stride kernels)
+  std::set<const void*> smem_opted;   // kernels whose >48 KB dynamic shared memory opt-in is done for this handle
   int64_t launches = 0;   // kernels launched through this handle
   Timer timer;
 };
@@ -83,10 +102,12 @@ template <class R> void launch_pack(const Grid<R>& g, const R* valid_src, R* pad
 template <class R> void launch_unpack(const Grid<R>& g, const R* padded_src, R* valid_dst, Ctx& c);
 
 // ---- particles.cu
-enum { kDepositGlobal = 1, kDepositCoop = 2, kDepositTile = 3, kDepositTileMma = 4 };
+enum { kDepositGlobal = 1, kDepositCoop = 2, kDepositTile = 3, kDepositTileMma = 4, kDepositFused = 5 };
 constexpr int kPushTileThreads = 256;   // k_push_tile: threads per CTA (one CTA per tile)
 constexpr int kDepMmaWarps = 4;         // k_deposit_mma: warps per CTA (one CTA per tile) ...
 constexpr int kDepMmaCtas = 5;          // ... and CTAs per SM the register budget is set for (20 warps per SM)
+constexpr int kFusedWarps = 12;         // k_fused_mma: warps per CTA (one CTA per tile, one per SM: box + 12 record buffers = 216 KB)
+constexpr int kFusedMaxDrift = 1024;    // ... and the drifted particles a CTA lists for its second pass
 constexpr int kDepTileWarps = 8;        // k_deposit_tile: warps per CTA (one CTA per tile, two per SM)
 template <class R>
 struct ParticleStep {
@@ -96,8 +117,7 @@ struct ParticleStep {
   const int32_t* tile_start;         // TILE: first slot of every tile (n_tiles + 1 entries)
   TileSpec tiles;
   int32_t* stray_list;               // scratch: indices a kernel hands to the next one (capacity n)
-  int32_t* stray_list2;
-  unsigned int* stray_count;         // [0] entries of stray_list, [1] of stray_list2
+  unsigned int* stray_count;         // entries of stray_list
   unsigned long long* deactivated;
 };
 // One particle step of a species. Returns true if the new positions are in alt.{x,y,z}
@@ -105,10 +125,11 @@ struct ParticleStep {
 template <class R>
 bool launch_particles(const Grid<R>& g, const ParticleStep<R>& a, int order, int mode, Ctx& c);
 
-// ---- tile_kernels.cu: k_push_tile + k_deposit_tile of one species (needs tile_start); particles
-// they could not finish are in stray_list / stray_count[0]
+// ---- tile_kernels.cu: the tile kernels of one species (needs tile_start): k_push_tile + k_deposit_tile /
+// k_deposit_mma, or k_fused_mma (mode = kDepositTile / kDepositTileMma / kDepositFused); particles they
+// could not finish are in stray_list / stray_count[0]
 template <class R>
-void launch_tile_kernels(const Grid<R>& g, const ParticleStep<R>& a, int order, bool mma, Ctx& c);
+void launch_tile_kernels(const Grid<R>& g, const ParticleStep<R>& a, int order, int mode, Ctx& c);
 
 // ---- sort.cu
 struct SortScratch {
@@ -120,8 +141,7 @@ struct SortScratch {
   int64_t hist_len = 0;
   int64_t scan_len = 0;
   int32_t* stray_list = nullptr;  // particles.cu: indices handed from one deposition kernel to the next
-  int32_t* stray_list2 = nullptr;
-  unsigned int* stray_count = nullptr;   // two counters
+  unsigned int* stray_count = nullptr;
 };
 int64_t sort_chunk();                                  // keys per block of a radix pass
 int64_t sort_hist_len(int64_t n);                      // entries of `hist` for n particles

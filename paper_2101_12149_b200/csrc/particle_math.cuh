@@ -20,19 +20,19 @@ __device__ __forceinline__ R interp(const R* __restrict__ F, int base, int sy, i
 #pragma unroll
         for (int a = 0; a <= ORDER; ++a)
           acc = add_rn(acc, mul_rn(mul_rn(mul_rn(wx[a], wy[b]), wz[c]), __ldg(F + base + a + sy * b + sz * c)));
-    return acc;
-  }
+  } else {
 #pragma unroll
-  for (int c = 0; c <= ORDER; ++c) {
-    R accb = 0;
+    for (int c = 0; c <= ORDER; ++c) {
+      R accb = 0;
 #pragma unroll
-    for (int b = 0; b <= ORDER; ++b) {
-      R acca = 0;
+      for (int b = 0; b <= ORDER; ++b) {
+        R acca = 0;
 #pragma unroll
-      for (int a = 0; a <= ORDER; ++a) acca += wx[a] * __ldg(F + base + a + sy * b + sz * c);
-      accb += wy[b] * acca;
+        for (int a = 0; a <= ORDER; ++a) acca += wx[a] * __ldg(F + base + a + sy * b + sz * c);
+        accb += wy[b] * acca;
+      }
+      acc += wz[c] * accb;
     }
-    acc += wz[c] * accb;
   }
   return acc;
 }

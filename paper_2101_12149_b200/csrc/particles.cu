@@ -107,8 +107,6 @@ template <class R, int ORDER>
 __global__ void __launch_bounds__(kCoopWarps * 32) k_deposit_coop(Grid<R> g, Particles<R> p, R* __restrict__ xn,
                                                                   R* __restrict__ yn, R* __restrict__ zn,
                                                                   const int32_t* __restrict__ cell_sorted,
-                                                                  const int32_t* __restrict__ in_list,
-                                                                  const unsigned int* __restrict__ in_count,
                                                                   int32_t* __restrict__ stray_list,
                                                                   unsigned int* __restrict__ stray_count,
                                                                   unsigned long long* deactivated) {
@@ -160,14 +158,13 @@ __global__ void __launch_bounds__(kCoopWarps * 32) k_deposit_coop(Grid<R> g, Par
     cur_ib += 1;
   };
 
-  // direct: a warp walks kCoopChunk consecutive particles; list: the warps stride over the list
+  // a warp walks kCoopChunk consecutive particles
   const int64_t wg = (int64_t)blockIdx.x * kCoopWarps + warp;
-  const int64_t begin = in_list ? wg * 32 : wg * kCoopChunk;
-  const int64_t end = in_list ? (int64_t)*in_count : min(p.n, begin + kCoopChunk);
-  const int64_t step = in_list ? (int64_t)gridDim.x * kCoopWarps * 32 : 32;
-  for (int64_t b0 = begin; b0 < end; b0 += step) {
+  const int64_t begin = wg * kCoopChunk;
+  const int64_t end = min(p.n, begin + kCoopChunk);
+  for (int64_t b0 = begin; b0 < end; b0 += 32) {
     const bool valid = b0 + lane < end;
-    const int64_t t = valid ? (in_list ? (int64_t)in_list[b0 + lane] : b0 + lane) : 0;
+    const int64_t t = valid ? b0 + lane : 0;
     bool elig = false;
     int ib = 0;
     R x1[3] = {0, 0, 0};
@@ -356,7 +353,7 @@ template <class R, int ORDER>
 bool launch_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) {
   const Particles<R>& p = a.cur;
   if (p.n == 0) return false;
-  if (mode != kDepositCoop && mode != kDepositTile && mode != kDepositTileMma) {
+  if (mode == kDepositGlobal) {
     ScopedPhase ph(c, kPhasePush);
     int64_t nb = (p.n + 127) / 128;
     k_particles_global<R, ORDER><<<(unsigned)nb, 128, 0, c.stream>>>(g, p, a.deactivated);
@@ -364,20 +361,13 @@ bool launch_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) 
     return false;
   }
   R *xn = a.alt.x, *yn = a.alt.y, *zn = a.alt.z;
-  const size_t smem = (size_t)kCoopWarps * 32 * Win<ORDER>::REC * sizeof(R);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(k_deposit_coop<R, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr_set = true;
-  }
-  if (mode == kDepositTile || mode == kDepositTileMma) {
-    // tile kernels, then the particles they listed: warp-cooperative pass over the list (window
-    // fixed to each particle's own cell), then one thread each for what that pass lists
-    cudaMemsetAsync(a.stray_count, 0, 2 * sizeof(unsigned int), c.stream);
-    launch_tile_kernels<R>(g, a, ORDER, mode == kDepositTileMma, c);
+  cudaMemsetAsync(a.stray_count, 0, sizeof(unsigned int), c.stream);
+  if (mode == kDepositTile || mode == kDepositTileMma || mode == kDepositFused) {
+    // tile kernels, then the particles they listed, one warp each
+    launch_tile_kernels<R>(g, a, ORDER, mode, c);
     ScopedPhase ph(c, kPhaseStray);
-    k_deposit_list_warp<R, ORDER><<<148 * 64, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count,
-                                                                 a.deactivated);
+    k_deposit_list_warp<R, ORDER><<<c.sm_count * 64, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list,
+                                                                        a.stray_count, a.deactivated);
     c.launches += 1;
     return true;
   }
@@ -385,17 +375,19 @@ bool launch_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) 
     ScopedPhase ph(c, kPhasePush);
     k_push<R, ORDER><<<(unsigned)((p.n + 127) / 128), 128, 0, c.stream>>>(g, p, xn, yn, zn);
   }
-  cudaMemsetAsync(a.stray_count, 0, sizeof(unsigned int), c.stream);
+  const size_t smem = (size_t)kCoopWarps * 32 * Win<ORDER>::REC * sizeof(R);
+  if (c.smem_opted.insert((const void*)k_deposit_coop<R, ORDER>).second)
+    cudaFuncSetAttribute(k_deposit_coop<R, ORDER>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   const int64_t per_cta = (int64_t)kCoopWarps * kCoopChunk;
   {
     ScopedPhase ph(c, kPhaseDeposit);
     k_deposit_coop<R, ORDER><<<(unsigned)((p.n + per_cta - 1) / per_cta), kCoopWarps * 32, smem, c.stream>>>(
-        g, p, xn, yn, zn, a.cell_sorted, nullptr, nullptr, a.stray_list, a.stray_count, a.deactivated);
+        g, p, xn, yn, zn, a.cell_sorted, a.stray_list, a.stray_count, a.deactivated);
   }
   {
     ScopedPhase ph(c, kPhaseStray);
-    k_deposit_list<R, ORDER><<<148 * 4, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count,
-                                                            a.deactivated);
+    k_deposit_list<R, ORDER><<<c.sm_count * 4, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count,
+                                                                   a.deactivated);
   }
   c.launches += 3;
   return true;

@@ -135,6 +135,8 @@ struct Sim : SimBase {
     sort_interval = o.sort_interval;
     deposit_mode = o.deposit_mode;
     ctx.stream = (cudaStream_t)o.cuda_stream;
+    PIC_CUDA(cudaGetDevice(&ctx.device));
+    PIC_CUDA(cudaDeviceGetAttribute(&ctx.sm_count, cudaDevAttrMultiProcessorCount, ctx.device));
     int64_t tot = 1;
     for (int d = 0; d < 3; ++d) {
       dx[d] = dx_[d];
@@ -227,7 +229,6 @@ struct Sim : SimBase {
     pool.free(scratch.hist);
     pool.free(scratch.scan_tmp);
     pool.free(scratch.stray_list);
-    pool.free(scratch.stray_list2);
     pool.free(scratch.stray_count);
     scratch = SortScratch();
     scratch.hist_len = sort_hist_len(n);
@@ -240,9 +241,8 @@ struct Sim : SimBase {
     scratch.hist = palloc<uint32_t>((size_t)scratch.hist_len);
     scratch.scan_tmp = palloc<uint32_t>((size_t)scratch.scan_len);
     scratch.stray_list = palloc<int32_t>((size_t)n);
-    scratch.stray_list2 = palloc<int32_t>((size_t)n);
-    scratch.stray_count = palloc<unsigned int>(2);
-    if (!scratch.hist || !scratch.scan_tmp || !scratch.stray_list || !scratch.stray_list2 || !scratch.stray_count)
+    scratch.stray_count = palloc<unsigned int>(1);
+    if (!scratch.hist || !scratch.scan_tmp || !scratch.stray_list || !scratch.stray_count)
       return fail(PIC_ERR_OOM, "sort scratch allocation failed");
     scratch.cap = n;
     return PIC_OK;
@@ -346,16 +346,20 @@ struct Sim : SimBase {
     }
   }
 
-  // AUTO: the warp-cooperative deposition needs the cell-sorted order to pay off
+  // AUTO: the tile kernels need the cell-sorted order, bins of at most 8 cells per axis and (unless asked
+  // for) enough cells per tile to pay for a CTA; until the first sort the fused per-particle kernel runs
   int pick_mode(const Species<R>& sp) const {
-    // the tile kernels want bins of at most 8 cells per axis and enough cells to pay for a CTA
     const bool tiles_ok = sp.sorted_once && tile.T[0] <= 8 && tile.T[1] <= 8 && tile.T[2] <= 8 &&
                           (deposit_mode != PIC_DEPOSIT_AUTO || tile.T[0] * tile.T[1] * tile.T[2] >= 64);
-    const bool want_tile = deposit_mode == PIC_DEPOSIT_TILE || deposit_mode == PIC_DEPOSIT_TILE_MMA;
+    const bool want_tile = deposit_mode == PIC_DEPOSIT_TILE || deposit_mode == PIC_DEPOSIT_TILE_MMA ||
+                           deposit_mode == PIC_DEPOSIT_FUSED;
     if (want_tile && !tiles_ok) return sp.sorted_once ? kDepositCoop : kDepositGlobal;
+    // fp32 has no fused kernel (its contraction is the fp64 tensor pipe's): the split tile kernels
+    if (deposit_mode == PIC_DEPOSIT_FUSED && sizeof(R) == 4) return kDepositTile;
     if (deposit_mode != PIC_DEPOSIT_AUTO) return deposit_mode;
-    // fp64: the tensor-pipe deposition; fp32: the lane-group one (its sums run on the fp32 pipe)
-    const int tile_mode = sizeof(R) == 8 ? kDepositTileMma : kDepositTile;
+    // fp64: gather + push + tensor-pipe deposition in one kernel; fp32: push, then the lane-group deposition
+    // (its sums run on the fp32 pipe)
+    const int tile_mode = sizeof(R) == 8 ? kDepositFused : kDepositTile;
     return tiles_ok ? tile_mode : (sp.sorted_once ? kDepositCoop : kDepositGlobal);
   }
   void particle_step(Species<R>& sp) {
@@ -366,7 +370,6 @@ struct Sim : SimBase {
     a.tile_start = sp.tile_start;
     a.tiles = tile;
     a.stray_list = scratch.stray_list;
-    a.stray_list2 = scratch.stray_list2;
     a.stray_count = scratch.stray_count;
     a.deactivated = d_deact;
     if (launch_particles<R>(g, a, order, pick_mode(sp), ctx)) {
@@ -412,7 +415,7 @@ struct Sim : SimBase {
         launch_fill_guards<R>(g, g.F, 6, ctx);       // FillBoundary
       }
       step_count++;
-      if (ctx.timer.spans.size() > 3000) ctx.timer.fold();
+      if (ctx.timer.spans.size() > 3000) ctx.timer.fold_completed();   // never waits: pic_step stays asynchronous
     }
     step_launches += ctx.launches - launches0;
     return check_launch("pic_step launch");
@@ -499,18 +502,21 @@ struct Sim : SimBase {
     size_t nv = (size_t)g.N[0] * g.N[1] * g.N[2];
     double* rho = palloc<double>(nv);
     if (!rho) return fail(PIC_ERR_OOM, "rho allocation failed");
-    PIC_CUDA(cudaMemsetAsync(d_red, 0, 8 * sizeof(double), ctx.stream));
-    launch_field_energy<R>(g, d_red, ctx);
-    for (auto& sp : species) launch_particle_sums<R>(sp.buf[sp.cur], sp.q, sp.m, d_red + 2, ctx);
-    int rc = fill_rho(rho);
-    if (rc) { pool.free(rho); return rc; }
-    launch_gauss<R>(g, rho, d_red + 4, ctx);
     double h[8];
     unsigned long long deact = 0;
+    // the pool block goes back on every path (stream order makes an immediate free safe)
+    int rc = [&]() -> int {
+      PIC_CUDA(cudaMemsetAsync(d_red, 0, 8 * sizeof(double), ctx.stream));
+      launch_field_energy<R>(g, d_red, ctx);
+      for (auto& sp : species) launch_particle_sums<R>(sp.buf[sp.cur], sp.q, sp.m, d_red + 2, ctx);
+      int r = fill_rho(rho);
+      if (r) return r;
+      launch_gauss<R>(g, rho, d_red + 4, ctx);
+      PIC_CUDA(cudaMemcpyAsync(h, d_red, sizeof(h), cudaMemcpyDeviceToHost, ctx.stream));
+      PIC_CUDA(cudaMemcpyAsync(&deact, d_deact, sizeof(deact), cudaMemcpyDeviceToHost, ctx.stream));
+      return sync();
+    }();
     pool.free(rho);
-    PIC_CUDA(cudaMemcpyAsync(h, d_red, sizeof(h), cudaMemcpyDeviceToHost, ctx.stream));
-    PIC_CUDA(cudaMemcpyAsync(&deact, d_deact, sizeof(deact), cudaMemcpyDeviceToHost, ctx.stream));
-    rc = sync();
     if (rc) return rc;
     double dv = dx[0] * dx[1] * dx[2];
     out[PIC_DIAG_FIELD_E] = 0.5 * kEps0 * h[0] * dv;
@@ -599,7 +605,7 @@ int pic_create(const int32_t n_cells[3], const double dx[3], double dt, int shap
   if (shape_order < 1 || shape_order > 3) return bad(PIC_ERR_INVALID_ARG, "shape_order must be 1, 2 or 3");
   if (prec != PIC_F64 && prec != PIC_F32) return bad(PIC_ERR_INVALID_ARG, "unknown precision");
   if (o.sort_interval < 0 || o.sort_key_mode < 0 || o.sort_key_mode > 1 || o.deposit_mode < 0 ||
-      o.deposit_mode > 4 || o.pusher < 0 || o.pusher > 1 || o.gather_mode < 0 || o.gather_mode > 1 ||
+      o.deposit_mode > 5 || o.pusher < 0 || o.pusher > 1 || o.gather_mode < 0 || o.gather_mode > 1 ||
       o.solver < 0 || o.solver > 1)
     return bad(PIC_ERR_INVALID_ARG, "bad option value");
   double s2 = 0;

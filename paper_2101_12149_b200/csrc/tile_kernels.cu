@@ -76,19 +76,19 @@ __device__ __forceinline__ R interp_box(const R* __restrict__ F, int base, const
 #pragma unroll
         for (int a = 0; a < NX; ++a)
           acc = add_rn(acc, mul_rn(mul_rn(mul_rn(wx[a], wy[b]), wz[c]), F[base + SX * a + b + E * c]));
-    return acc;
-  }
+  } else {
 #pragma unroll
-  for (int c = 0; c < NZ; ++c) {
-    R accb = 0;
+    for (int c = 0; c < NZ; ++c) {
+      R accb = 0;
 #pragma unroll
-    for (int b = 0; b < NY; ++b) {
-      R acca = 0;
+      for (int b = 0; b < NY; ++b) {
+        R acca = 0;
 #pragma unroll
-      for (int a = 0; a < NX; ++a) acca += wx[a] * F[base + SX * a + b + E * c];
-      accb += wy[b] * acca;
+        for (int a = 0; a < NX; ++a) acca += wx[a] * F[base + SX * a + b + E * c];
+        accb += wy[b] * acca;
+      }
+      acc += wz[c] * accb;
     }
-    acc += wz[c] * accb;
   }
   return acc;
 }
@@ -221,9 +221,8 @@ struct TWin {
 // and 3 the old support starts at a fixed slot (cell - 1 + ... is static), so only the new weights
 // need selects.
 template <class R, int ORDER, int NW, int BL>
-__device__ __forceinline__ void axis_window(R xi0, R xi1, int& cell, R* S0, R* DS, bool& fits) {
-  R w0[ORDER + 1], w1[ORDER + 1];
-  const int l0 = shape<R, ORDER>(xi0, w0);
+__device__ __forceinline__ void axis_window_from(int l0, const R* w0, R xi0, R xi1, int& cell, R* S0, R* DS, bool& fits) {
+  R w1[ORDER + 1];
   const int l1 = shape<R, ORDER>(xi1, w1);
   const int c = ORDER == 2 ? (int)floor(xi0) : (ORDER == 1 ? l0 : l0 + 1);
   cell = c;
@@ -264,6 +263,13 @@ __device__ __forceinline__ void axis_window(R xi0, R xi1, int& cell, R* S0, R* D
     DS[i] = sub_rn(b, a);
   }
   fits = (so0 >= 0) & (so0 + ORDER < NW) & (sl1 >= 0) & (sl1 + ORDER < NW);
+}
+
+template <class R, int ORDER, int NW, int BL>
+__device__ __forceinline__ void axis_window(R xi0, R xi1, int& cell, R* S0, R* DS, bool& fits) {
+  R w0[ORDER + 1];
+  const int l0 = shape<R, ORDER>(xi0, w0);
+  axis_window_from<R, ORDER, NW, BL>(l0, w0, xi0, xi1, cell, S0, DS, fits);
 }
 
 
@@ -733,14 +739,329 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
   if (cur != INT_MIN) retire_rows(false, 0);
 }
 
+// =================================================================== gather + push + deposit, one kernel (fp64)
+// PAPER.md:114 argues for fusing the gather into the push so that no per-particle field ever reaches
+// memory; the same argument holds one step further: the deposit needs x_old, x_new, w and the nodal
+// weights of x_old, all of which the push has in registers. Here one CTA per tile stages the E/B box
+// (as k_push_tile) and each warp takes rounds of 32 particles through the whole particle step: lane =
+// particle for gather + push + the deposit's per-axis record, then the warp contracts the round's records
+// on the fp64 tensor pipe (as k_deposit_mma). x_new goes to memory once, wrapped; x_old, w and the record
+// never do. The gather is bound by shared-memory wavefronts and the contraction by the fp64 pipe, so warps
+// in different phases of their rounds fill each other's idle unit on the same SM.
+// Particles that drifted out of the tile's box since the last sort are listed and taken through the same
+// code in a second pass that gathers from global memory (all lanes busy); particles whose move does not
+// fit the deposit windows (cell change in y or z) are pushed here and listed for k_deposit_list_warp.
+template <int ORDER, int PUSHER, int GATHER, int NWARP>
+__global__ void __launch_bounds__(NWARP * 32, 1)
+    k_fused_mma(Grid<double> g, Particles<double> p, double* __restrict__ xn, double* __restrict__ yn,
+                double* __restrict__ zn, const int32_t* __restrict__ tile_start, TileSpec ts,
+                int32_t* __restrict__ stray_list, unsigned int* __restrict__ stray_count,
+                unsigned long long* deactivated) {
+  using R = double;
+  using PB = PushBox<ORDER>;
+  using W = MWin<ORDER>;
+  constexpr int E = PB::EXT, SX = PB::SX, VOL = PB::VOL;
+  constexpr int NS = GATHER == 1 ? ORDER : ORDER + 1;   // weights along a staggered axis
+  constexpr int NN = ORDER + 1;
+  constexpr int NX = W::NX, NYZ = W::NYZ, NB = W::NB, REC = W::REC, BLX = W::BLX, BLYZ = W::BLYZ;
+  constexpr int MAXD = kFusedMaxDrift;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  R* box = reinterpret_cast<R*>(smem_raw);   // [6][E (x)][SX: E (z) x E (y), padded]
+  R* rec_all = box + 6 * VOL;
+  __shared__ int s_drift[MAXD];
+  __shared__ int s_ndrift;
+
+  const int tile = blockIdx.x;
+  const int s = tile_start[tile], e = tile_start[tile + 1];
+  if (s >= e) return;
+  if (threadIdx.x == 0) s_ndrift = 0;
+  int tb[3];
+  tile_coords(ts, tile, tb);
+  const int o0 = tb[0] - PB::HB, o1 = tb[1] - PB::HB, o2 = tb[2] - PB::HB;   // node of local (0,0,0)
+  {
+    const int lim0 = g.N[0] + kGuard, lim1 = g.N[1] + kGuard, lim2 = g.N[2] + kGuard;
+    for (int idx = threadIdx.x; idx < E * E * E; idx += blockDim.x) {
+      int i = idx % E, r = idx / E;
+      int j = r % E, k = r / E;
+      const bool in = (o0 + i < lim0) & (o1 + j < lim1) & (o2 + k < lim2);
+      const int gi = g.idx(o0 + i, o1 + j, o2 + k);
+      const int li = SX * i + j + E * k;
+#pragma unroll
+      for (int c = 0; c < 6; ++c) {
+        if (in) cp_async(box + c * VOL + li, g.F[c] + gi);
+        else box[c * VOL + li] = R(0);
+      }
+    }
+  }
+
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int gq = lane >> 2, t = lane & 3;           // fragment coordinates of this lane
+  R* rec = rec_all + (size_t)warp * 33 * REC;       // 32 records of the round + one that stays zero
+  const R* zrec = rec + 32 * REC;
+  for (int i = lane; i < REC; i += 32) rec[32 * REC + i] = R(0);
+  const R half = R(0.5), third = R(1) / R(3);
+
+  // B operands: this lane supplies column gq (+ 8 per block) = (jB, kB + KSTEP * block)
+  const bool colok = gq < W::NCOL;
+  const int jB = colok ? gq % NYZ : 0, kB = colok ? gq / NYZ : 0;
+  const int offY = W::oY + 2 * jB, offPY = W::oPY + jB, offZ = W::oZ + 2 * kB, offPZ = W::oPZ + kB;
+  // C fragments: this lane holds columns 2t + {0,1} (+ 8 per block) of row gq
+  int coff[NB][2];
+  bool cok[NB][2];
+#pragma unroll
+  for (int b = 0; b < NB; ++b)
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      const int n = 2 * t + c + 8 * b;
+      cok[b][c] = n < W::NCOL;
+      coff[b][c] = (n % NYZ) * g.sy + (n / NYZ) * g.sz;
+    }
+
+  CFrag<NB> C;
+  C.zero();
+  int cur = INT_MIN;   // packed cell triple of the window being accumulated
+  auto win_x = [&](int cd) { return tb[0] + 3 * (cd & 15) - 4 - BLX; };   // first node of a triple's 8-node window
+  auto win_y = [&](int cd) { return tb[1] + ((cd >> 4) & 15) - 4 - BLYZ; };
+  auto win_z = [&](int cd) { return tb[2] + (cd >> 8) - 4 - BLYZ; };
+  auto retire_rows = [&](bool same_row, int nx0) {
+    const int ox0 = win_x(cur);
+    const int io = (gq - ox0) & 7;
+    const int X = ox0 + io;
+    const bool keep = same_row && X >= nx0 && X < nx0 + 8;
+    if (!keep) {
+      const int base = g.idx(X, win_y(cur), win_z(cur));
+#pragma unroll
+      for (int b = 0; b < NB; ++b)
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+          if (cok[b][c]) {
+            if (C.x[b][c] != 0.0) red_add(g.J[0] + base + coff[b][c], C.x[b][c]);
+            if (C.y[b][c] != 0.0) red_add(g.J[1] + base + coff[b][c], C.y[b][c]);
+            if (C.z[b][c] != 0.0) red_add(g.J[2] + base + coff[b][c], C.z[b][c]);
+          }
+          C.x[b][c] = 0; C.y[b][c] = 0; C.z[b][c] = 0;
+        }
+    }
+  };
+
+  // the warp's contiguous share of the tile: whole rounds of 32, sizes differing by at most one round
+  const int n = e - s;
+  const int rounds = (n + 31) >> 5;
+  const int wb = s + 32 * (int)(((long long)rounds * warp) / NWARP);
+  const int we = min(e, s + 32 * (int)(((long long)rounds * (warp + 1)) / NWARP));
+
+  asm volatile("cp.async.wait_all;" ::: "memory");
+  __syncthreads();
+
+#pragma unroll 1
+  for (int phase = 0; phase < 2; ++phase) {
+    int r_begin = wb, r_end = we, r_step = 32;
+    if (phase == 1) {
+      __syncthreads();                                   // every warp's drifted particles are listed
+      r_begin = 32 * warp;
+      r_end = min(s_ndrift, MAXD);
+      r_step = 32 * NWARP;
+    }
+#pragma unroll 1
+    for (int rb = r_begin; rb < r_end; rb += r_step) {
+      bool valid = rb + lane < r_end;
+      int tp = rb + lane;
+      if (phase == 1) tp = valid ? s_drift[tp] : 0;
+      bool elig = false;
+      R x1[3] = {0, 0, 0};
+      R w = 0;
+      int code = -1;
+      if (phase == 0 && tp + 32 < we) {   // the next round's particle data on its way to L2
+        prefetch_l2(p.x + tp + 32); prefetch_l2(p.y + tp + 32); prefetch_l2(p.z + tp + 32);
+        prefetch_l2(p.ux + tp + 32); prefetch_l2(p.uy + tp + 32); prefetch_l2(p.uz + tp + 32);
+        prefetch_l2(p.w + tp + 32);
+      }
+      if (valid) {
+        const R x0[3] = {p.x[tp], p.y[tp], p.z[tp]};
+        R u[3] = {p.ux[tp], p.uy[tp], p.uz[tp]};
+        w = p.w[tp];
+        R wn[3][ORDER + 1], xi0[3];
+        int ln[3];
+        R Ef[3], Bf[3];
+        bool inbox = phase == 0;
+        {
+          R ws[3][ORDER + 1];
+          int ls[3];
+#pragma unroll
+          for (int d = 0; d < 3; ++d) {
+            xi0[d] = mul_rn(x0[d], g.inv_dx[d]);
+            const R xs = sub_rn(xi0[d], R(0.5));
+            const int od = d == 0 ? o0 : (d == 1 ? o1 : o2);
+            ln[d] = shape<R, ORDER>(xi0[d], wn[d]);
+            ls[d] = (GATHER == 1 ? shape_lowered<R, ORDER>(xs, ws[d]) : shape<R, ORDER>(xs, ws[d])) - od;
+            const int lr = ln[d] - od;
+            inbox &= (lr >= 0) & (lr <= E - ORDER - 1) & (ls[d] >= 0) & (ls[d] <= E - ORDER - 1);
+          }
+          if (inbox) {
+            const int l0 = ln[0] - o0, l1 = ln[1] - o1, l2 = ln[2] - o2;
+            // Ex (s,n,n)  Ey (n,s,n)  Ez (n,n,s)  Bx (n,s,s)  By (s,n,s)  Bz (s,s,n)
+            Ef[0] = interp_box<R, ORDER, NS, NN, NN>(box + 0 * VOL, SX * ls[0] + l1 + E * l2, ws[0], wn[1], wn[2]);
+            Ef[1] = interp_box<R, ORDER, NN, NS, NN>(box + 1 * VOL, SX * l0 + ls[1] + E * l2, wn[0], ws[1], wn[2]);
+            Ef[2] = interp_box<R, ORDER, NN, NN, NS>(box + 2 * VOL, SX * l0 + l1 + E * ls[2], wn[0], wn[1], ws[2]);
+            Bf[0] = interp_box<R, ORDER, NN, NS, NS>(box + 3 * VOL, SX * l0 + ls[1] + E * ls[2], wn[0], ws[1], ws[2]);
+            Bf[1] = interp_box<R, ORDER, NS, NN, NS>(box + 4 * VOL, SX * ls[0] + l1 + E * ls[2], ws[0], wn[1], ws[2]);
+            Bf[2] = interp_box<R, ORDER, NS, NS, NN>(box + 5 * VOL, SX * ls[0] + ls[1] + E * l2, ws[0], ws[1], wn[2]);
+          }
+        }
+        if (!inbox) {
+          // drifted out of the tile's box since the last sort: second pass (gather from global memory with all
+          // lanes busy); in line if the list is full
+          int slot = MAXD;
+          if (phase == 0) slot = atomicAdd(&s_ndrift, 1);
+          if (slot < MAXD) {
+            s_drift[slot] = tp;
+            valid = false;
+          } else {
+            gather6<R, ORDER, GATHER != 0>(g, x0[0], x0[1], x0[2], Ef, Bf);
+          }
+        }
+        if (valid) {
+          push_momentum<R>(PUSHER, p.kq, g.inv_c2, Ef, Bf, u);
+          advance<R>(g.dt, g.inv_c2, x0, u, x1);
+          p.ux[tp] = u[0]; p.uy[tp] = u[1]; p.uz[tp] = u[2];
+          R S0x[NX], DSx[NX], S0y[NYZ], DSy[NYZ], S0z[NYZ], DSz[NYZ];
+          int c[3];
+          bool fit[3];
+          axis_window_from<R, ORDER, NX, BLX>(ln[0], wn[0], xi0[0], mul_rn(x1[0], g.inv_dx[0]), c[0], S0x, DSx, fit[0]);
+          axis_window_from<R, ORDER, NYZ, BLYZ>(ln[1], wn[1], xi0[1], mul_rn(x1[1], g.inv_dx[1]), c[1], S0y, DSy, fit[1]);
+          axis_window_from<R, ORDER, NYZ, BLYZ>(ln[2], wn[2], xi0[2], mul_rn(x1[2], g.inv_dx[2]), c[2], S0z, DSz, fit[2]);
+          // the cell must be inside the grid and within 4 cells of the tile (4-bit biased offsets)
+          const int rc0 = c[0] - tb[0] + 4, rc1 = c[1] - tb[1] + 4, rc2 = c[2] - tb[2] + 4;
+          elig = fit[0] & fit[1] & fit[2] & (((rc0 | rc1 | rc2) & ~15) == 0) & (c[0] >= 0) & (c[0] < g.N[0]) &
+                 (c[1] >= 0) & (c[1] < g.N[1]) & (c[2] >= 0) & (c[2] < g.N[2]);
+          if (elig) {
+            code = rc0 | (rc1 << 4) | (rc2 << 8);
+            R* rr = rec + lane * REC;
+            const R fx = -(w * p.jf[0]), fy = -(w * p.jf[1]), fz = -(w * p.jf[2]);
+            R px = 0, py = 0, pz = 0;
+#pragma unroll
+            for (int i = 0; i < NX; ++i) {
+              *reinterpret_cast<Pair2<R>*>(rr + W::oAB + 2 * i) =
+                  Pair2<R>{S0x[i] + half * DSx[i], half * S0x[i] + third * DSx[i]};
+              px += DSx[i];
+              rr[W::oPX + i] = fx * px;
+            }
+#pragma unroll
+            for (int i = 0; i < NYZ; ++i) {
+              *reinterpret_cast<Pair2<R>*>(rr + W::oY + 2 * i) = Pair2<R>{S0y[i], DSy[i]};
+              *reinterpret_cast<Pair2<R>*>(rr + W::oZ + 2 * i) = Pair2<R>{S0z[i], DSz[i]};
+              py += DSy[i]; pz += DSz[i];
+              rr[W::oPY + i] = fy * py;
+              rr[W::oPZ + i] = fz * pz;
+            }
+          }
+        }
+      }
+      __syncwarp();
+      // runs of consecutive particles whose cells lie in the same triple of x-neighbouring cells of one
+      // (y,z) row share the accumulators (see k_deposit_mma). Warp-uniform control flow.
+      const int scode = code < 0 ? -1 : ((code & ~15) | ((code & 15) / 3));
+      const int prev = __shfl_up_sync(0xffffffffu, scode, 1);
+      unsigned heads = __ballot_sync(0xffffffffu, lane == 0 || scode != prev);
+      const unsigned live = __ballot_sync(0xffffffffu, code >= 0);
+      while (heads) {
+        const int s0 = __ffs(heads) - 1;
+        heads &= heads - 1;
+        const int s1 = heads ? __ffs(heads) - 1 : 32;
+        if (!((live >> s0) & 1u)) continue;
+        const int cd = __shfl_sync(0xffffffffu, scode, s0);
+        if (cd != cur) {
+          if (cur != INT_MIN) retire_rows(((cd ^ cur) >> 4) == 0, win_x(cd));
+          cur = cd;
+        }
+#pragma unroll 2
+        for (int b = s0; b < s1; b += 4) {
+          const bool here = b + t < s1;
+          const int pc = __shfl_sync(0xffffffffu, code, (b + t) & 31);
+          const int i = (gq - (tb[0] + (pc & 15) - 4 - BLX)) & 7;      // window slot of this lane's row
+          const bool rowok = i < NX;
+          const R* rr = rec + (here ? b + t : 32) * REC;               // slot 32: the all-zero record
+          const R* ra = rowok ? rr : zrec;
+          const double px = ra[W::oPX + (rowok ? i : 0)];
+          const Pair2<R> ab = *reinterpret_cast<const Pair2<R>*>(ra + W::oAB + 2 * (rowok ? i : 0));
+          const Pair2<R> yv = *reinterpret_cast<const Pair2<R>*>(rr + offY);
+          const double py = colok ? (double)rr[offPY] : 0.0;
+          const double y0 = colok ? (double)yv.a : 0.0, y1 = colok ? (double)yv.b : 0.0;
+          const double al = fma(0.5, y1, y0), be = fma(0.5, y0, y1 * (1.0 / 3.0));
+#pragma unroll
+          for (int nb = 0; nb < NB; ++nb) {
+            const Pair2<R> zv = *reinterpret_cast<const Pair2<R>*>(rr + offZ + 2 * W::KSTEP * nb);
+            const double pz = rr[offPZ + W::KSTEP * nb];
+            const double z0 = zv.a, z1 = zv.b;
+            dmma_884(C.x[nb][0], C.x[nb][1], px, fma(z0, al, z1 * be));
+            dmma_884(C.y[nb][0], C.y[nb][1], (double)ab.a, py * z0);
+            dmma_884(C.z[nb][0], C.z[nb][1], (double)ab.a, pz * y0);
+            dmma_884(C.y[nb][0], C.y[nb][1], (double)ab.b, py * z1);
+            dmma_884(C.z[nb][0], C.z[nb][1], (double)ab.b, pz * y1);
+          }
+        }
+      }
+      __syncwarp();
+      // particles deposited here are finished: wrap and store; the others are stored unwrapped and listed
+      const bool stray = valid && !elig;
+      const unsigned sm = __ballot_sync(0xffffffffu, stray);
+      if (sm) {
+        unsigned base = 0;
+        if (lane == 0) base = atomicAdd(stray_count, (unsigned)__popc(sm));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (stray) stray_list[base + __popc(sm & ((1u << lane) - 1u))] = (int32_t)tp;
+      }
+      if (valid) {
+        if (elig) {
+          bool out = false;
+#pragma unroll
+          for (int d = 0; d < 3; ++d) out |= wrap_axis<R>(x1[d], g.L[d], g.periodic[d]);
+          if (out) {
+            if (w != R(0)) atomicAdd(deactivated, 1ull);
+            p.w[tp] = R(0);
+          }
+        }
+        xn[tp] = x1[0]; yn[tp] = x1[1]; zn[tp] = x1[2];
+      }
+    }
+  }
+  if (cur != INT_MIN) retire_rows(false, 0);
+}
+
 }  // namespace
 
+// >48 KB of dynamic shared memory is an opt-in per function AND per device/context: done once per
+// simulation handle (Ctx), not once per process
+template <class K>
+static void opt_in_smem(Ctx& c, K kernel, size_t bytes) {
+  if (c.smem_opted.insert((const void*)kernel).second)
+    cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
+template <int ORDER>
+static void launch_fused(const Grid<double>& g, const ParticleStep<double>& a, Ctx& c) {
+  const Particles<double>& p = a.cur;
+  const int n_tiles = a.tiles.nt[0] * a.tiles.nt[1] * a.tiles.nt[2];
+  constexpr int NW = kFusedWarps;
+  const size_t smem = ((size_t)6 * PushBox<ORDER>::VOL + (size_t)NW * 33 * MWin<ORDER>::REC) * sizeof(double);
+  auto k = g.pusher == 0 ? (g.gather_mode == 0 ? k_fused_mma<ORDER, 0, 0, NW> : k_fused_mma<ORDER, 0, 1, NW>)
+                         : (g.gather_mode == 0 ? k_fused_mma<ORDER, 1, 0, NW> : k_fused_mma<ORDER, 1, 1, NW>);
+  opt_in_smem(c, k, smem);
+  ScopedPhase ph(c, kPhasePush);
+  k<<<n_tiles, NW * 32, smem, c.stream>>>(g, p, a.alt.x, a.alt.y, a.alt.z, a.tile_start, a.tiles, a.stray_list,
+                                           a.stray_count, a.deactivated);
+  c.launches += 1;
+}
+
 template <class R, int ORDER>
-static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, bool mma, Ctx& c) {
+static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) {
+  if constexpr (sizeof(R) == 8) {
+    if (mode == kDepositFused) { launch_fused<ORDER>(g, a, c); return; }
+  }
+  const bool mma = mode == kDepositTileMma;
   const Particles<R>& p = a.cur;
   R *xn = a.alt.x, *yn = a.alt.y, *zn = a.alt.z;
   const int n_tiles = a.tiles.nt[0] * a.tiles.nt[1] * a.tiles.nt[2];
-  static bool attr_set = false;
   constexpr int kW = kDepTileWarps;
   auto kvec = k_deposit_tile<R, ORDER, kW>;
   auto kmma = k_deposit_mma<R, ORDER, kDepMmaWarps, kDepMmaCtas>;
@@ -748,43 +1069,38 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, bool m
   const size_t push_smem = (size_t)6 * PushBox<ORDER>::VOL * sizeof(R);
   const size_t vec_smem = (size_t)kW * 32 * TWin<ORDER>::REC * sizeof(R);
   const size_t mma_smem = (size_t)mw * 33 * MWin<ORDER>::REC * sizeof(R);
-  if (!attr_set) {
-    cudaFuncSetAttribute(k_push_tile<R, ORDER, 0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
-    cudaFuncSetAttribute(k_push_tile<R, ORDER, 0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
-    cudaFuncSetAttribute(k_push_tile<R, ORDER, 1, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
-    cudaFuncSetAttribute(k_push_tile<R, ORDER, 1, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)push_smem);
-    cudaFuncSetAttribute(kvec, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vec_smem);
-    cudaFuncSetAttribute(kmma, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mma_smem);
-    attr_set = true;
-  }
   {
     ScopedPhase ph(c, kPhasePush);
     auto kpush = g.pusher == 0 ? (g.gather_mode == 0 ? k_push_tile<R, ORDER, 0, 0> : k_push_tile<R, ORDER, 0, 1>)
                                : (g.gather_mode == 0 ? k_push_tile<R, ORDER, 1, 0> : k_push_tile<R, ORDER, 1, 1>);
+    opt_in_smem(c, kpush, push_smem);
     kpush<<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles);
   }
   {
     ScopedPhase ph(c, kPhaseDeposit);
-    if (mma)
+    if (mma) {
+      opt_in_smem(c, kmma, mma_smem);
       kmma<<<n_tiles, mw * 32, mma_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
                                                     a.stray_count, a.deactivated);
-    else
+    } else {
+      opt_in_smem(c, kvec, vec_smem);
       kvec<<<n_tiles, kW * 32, vec_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
                                                     a.stray_count, a.deactivated);
+    }
   }
   c.launches += 2;
 }
 
 template <class R>
-void launch_tile_kernels(const Grid<R>& g, const ParticleStep<R>& a, int order, bool mma, Ctx& c) {
+void launch_tile_kernels(const Grid<R>& g, const ParticleStep<R>& a, int order, int mode, Ctx& c) {
   switch (order) {
-    case 1: launch_tile_order<R, 1>(g, a, mma, c); break;
-    case 2: launch_tile_order<R, 2>(g, a, mma, c); break;
-    default: launch_tile_order<R, 3>(g, a, mma, c); break;
+    case 1: launch_tile_order<R, 1>(g, a, mode, c); break;
+    case 2: launch_tile_order<R, 2>(g, a, mode, c); break;
+    default: launch_tile_order<R, 3>(g, a, mode, c); break;
   }
 }
 
-template void launch_tile_kernels<double>(const Grid<double>&, const ParticleStep<double>&, int, bool, Ctx&);
-template void launch_tile_kernels<float>(const Grid<float>&, const ParticleStep<float>&, int, bool, Ctx&);
+template void launch_tile_kernels<double>(const Grid<double>&, const ParticleStep<double>&, int, int, Ctx&);
+template void launch_tile_kernels<float>(const Grid<float>&, const ParticleStep<float>&, int, int, Ctx&);
 
 }  // namespace pic

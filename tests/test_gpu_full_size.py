@@ -96,14 +96,19 @@ def test_C4_full_size_sampled_parity_and_invariants():
     # (z-cells 128..192) and the electrons there are relativistic; step 101 does not sort
     g.step(100)
     p1 = g.get_particles(0)
-    E1, B1, _ = g.get_fields(with_J=False)
+    E1, B1, J1 = g.get_fields()
     assert max(np.max(np.abs(p1[k])) for k in ("ux", "uy", "uz")) > 0.3 * W.C_LIGHT
     cc = _cells(p1, cfg)
     zfront = int(cc[2].min()) - 3                     # no particle, hence no J, in the planes below this one
     assert zfront > 60
-    # (2) sub-boxes: in the ramp under the laser axis; across the end of the ramp, off axis; on the high z
-    # face in the periodic x-y corner (wraps in x and y, truncated in z)
-    boxes = [((58, 58, 150), (12, 12, 12)), ((30, 80, 186), (12, 12, 12)), ((-6, -6, 1012), (12, 12, 12))]
+    # (2) sub-boxes: around the strongest current of the previous step (the electrons the laser has swept up:
+    # on its axis they are blown out behind the front, so the place is taken from the data); in the ramp off
+    # axis; on the high z face in the periodic x-y corner (wraps in x and y, truncated in z)
+    kz, ky, kx = np.unravel_index(np.argmax(np.abs(J1[0])), J1[0].shape)
+    assert 128 <= kz < 400
+    del J1
+    boxes = [((int(kx) - 6, int(ky) - 6, int(kz) - 6), (12, 12, 12)), ((30, 80, 150), (12, 12, 12)),
+             ((-6, -6, 1012), (12, 12, 12))]
     margin = 3
     sel = np.zeros(len(cc[0]), dtype=bool)
     for lo, size in boxes:
@@ -135,8 +140,8 @@ def test_C4_full_size_sampled_parity_and_invariants():
             assert np.max(np.abs(Jg[c][ix] - Jo[c][ix])) <= TOL64 * jscale
             assert np.max(np.abs(Eg[c][ix] - Eo[c][ix])) <= TOL64 * escale
             assert np.max(np.abs(Bg[c][ix1] - Bo[c][ix1])) <= TOL64 * bscale
-        if bi < 2:
-            assert max(np.max(np.abs(Jo[c][ix])) for c in range(3)) > 1e-3 * jscale   # the laser drives J here
+        if bi == 0:
+            assert max(np.max(np.abs(Jo[c][ix])) for c in range(3)) > 0.1 * jscale    # the laser drives J here
     # in front of the plasma J is zero on both sides: the tail of the laser, what the plasma sent back and the
     # truncated low-z face evolve by the field solver alone and must match on every node
     assert all(np.all(Jg[c][:zfront] == 0) for c in range(3))

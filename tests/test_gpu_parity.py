@@ -77,7 +77,7 @@ def test_sort_edge_positions_and_ragged_sizes():
 
 # ------------------------------------------------------------------ one step from identical state
 @pytest.mark.parametrize("order", [1, 2, 3])
-@pytest.mark.parametrize("mode", [1, 2, 3, 4])
+@pytest.mark.parametrize("mode", [1, 2, 3, 4, 5])
 def test_one_step_fp64(order, mode):
     cfg = small("C2", (24, 16, 16), order=order, dx=(1.0e-6, 0.8e-6, 0.6e-6))
     cfg.species[0].sigma = 0.2            # hot: many cell crossings in one step
@@ -118,9 +118,10 @@ def test_fp32_push_is_bit_identical(order, mode, method):
 
 @pytest.mark.parametrize("order", [1, 2, 3])
 @pytest.mark.parametrize("tile", [(8, 8, 8), (4, 8, 2)])
-@pytest.mark.parametrize("mode", [3, 4])
+@pytest.mark.parametrize("mode", [3, 4, 5])
 def test_tile_path_steps_between_sorts(order, tile, mode):
-    """Tile kernels (one CTA per sort tile; deposition by lane groups = 3, on the fp64 tensor pipe = 4)
+    """Tile kernels (one CTA per sort tile; deposition by lane groups = 3, on the fp64 tensor pipe = 4, gather +
+    push + tensor-pipe deposition in one kernel = 5)
     on the steps after a sort, when hot particles have left their cell, the reach of their tile's
     windows (-> list -> per-particle pass) and its E/B box (-> drift list -> global gather)."""
     cfg = small("C2", (24, 16, 8), order=order, tile=tile, dx=(1.0e-6, 0.8e-6, 0.6e-6))
@@ -138,10 +139,11 @@ def test_tile_path_steps_between_sorts(order, tile, mode):
 # ------------------------------------------------------------------ SURVEY.md 8(f) NEXT-2 / NEXT-4
 @pytest.mark.parametrize("order", [1, 2, 3])
 @pytest.mark.parametrize("method", [dict(pusher=1), dict(gather_mode=1), dict(pusher=1, gather_mode=1)])
-@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("mode", [0, 1, 4])
 def test_vay_pusher_and_galerkin_gather_fp64(order, method, mode):
-    """Vay pusher / Galerkin gather on the tile path (mode 0, steps after the first sort,
-    drifted particles included) and on the fused per-particle kernel (mode 1); relativistic momenta so
+    """Vay pusher / Galerkin gather on the tile path (mode 0 = the one-kernel particle step,
+    mode 4 = push and deposit kernels; steps after the first sort, drifted particles included) and on the
+    per-particle kernel (mode 1); relativistic momenta so
     that the two pushers differ at first order."""
     cfg = small("C2", (24, 16, 16), order=order, dx=(1.0e-6, 0.8e-6, 0.6e-6))
     cfg.species[0].sigma = 0.6
@@ -232,7 +234,7 @@ def test_tile_path_fp32_steps_between_sorts():
     compare_state(o, g, 4 * TOL32)
 
 
-@pytest.mark.parametrize("mode", [3, 4])
+@pytest.mark.parametrize("mode", [3, 4, 5])
 def test_tile_path_empty_tiles_and_tile_only_key(mode):
     """Tiles with no particle (C4's vacuum region) and sort_key_mode 1 (order inside a tile is free)."""
     cfg = small("C4", (16, 16, 48), z_first=24, ramp_cells=8)
