@@ -76,12 +76,15 @@ enum {
                                  window node. AUTO picks this in fp32 when it can. */
   PIC_DEPOSIT_TILE_MMA = 4,   /* as TILE, but the sums of a cell's particles are formed as small
                                  dense contractions on the fp64 tensor pipe (mma.sync m8n8k4.f64),
-                                 one warp per cell run (fp64 arithmetic also for PIC_F32 data). */
+                                 one warp per cell run (fp64 arithmetic also for PIC_F32 data).
+                                 AUTO picks this in fp64 when it can. */
   PIC_DEPOSIT_FUSED = 5       /* gather + push + the TILE_MMA deposition in ONE kernel per species: a
                                  warp takes 32 particles through the whole particle step, so x_old,
                                  x_new, w and the nodal weights reach the deposit in registers and
                                  shared memory instead of through HBM. fp64 only (PIC_F32 runs TILE).
-                                 AUTO picks this in fp64 when it can. */
+                                 Measured slower than TILE_MMA's two kernels on B200 (one CTA of 12
+                                 warps per SM against 16 + 20 warps): kept
+                                 selectable, never picked by AUTO. */
 };
 
 /* Momentum update of step 2c. BORIS: the relativistic Boris rotation (BASELINE.json; DESIGN.md

@@ -357,9 +357,9 @@ struct Sim : SimBase {
     // fp32 has no fused kernel (its contraction is the fp64 tensor pipe's): the split tile kernels
     if (deposit_mode == PIC_DEPOSIT_FUSED && sizeof(R) == 4) return kDepositTile;
     if (deposit_mode != PIC_DEPOSIT_AUTO) return deposit_mode;
-    // fp64: gather + push + tensor-pipe deposition in one kernel; fp32: push, then the lane-group deposition
-    // (its sums run on the fp32 pipe)
-    const int tile_mode = sizeof(R) == 8 ? kDepositFused : kDepositTile;
+    // fp64: push, then the tensor-pipe deposition (the one-kernel form, PIC_DEPOSIT_FUSED, measured 9 % slower:
+    // DESIGN.md section 6); fp32: push, then the lane-group deposition (its sums run on the fp32 pipe)
+    const int tile_mode = sizeof(R) == 8 ? kDepositTileMma : kDepositTile;
     return tiles_ok ? tile_mode : (sp.sorted_once ? kDepositCoop : kDepositGlobal);
   }
   void particle_step(Species<R>& sp) {

@@ -139,10 +139,10 @@ def test_tile_path_steps_between_sorts(order, tile, mode):
 # ------------------------------------------------------------------ SURVEY.md 8(f) NEXT-2 / NEXT-4
 @pytest.mark.parametrize("order", [1, 2, 3])
 @pytest.mark.parametrize("method", [dict(pusher=1), dict(gather_mode=1), dict(pusher=1, gather_mode=1)])
-@pytest.mark.parametrize("mode", [0, 1, 4])
+@pytest.mark.parametrize("mode", [0, 1, 5])
 def test_vay_pusher_and_galerkin_gather_fp64(order, method, mode):
-    """Vay pusher / Galerkin gather on the tile path (mode 0 = the one-kernel particle step,
-    mode 4 = push and deposit kernels; steps after the first sort, drifted particles included) and on the
+    """Vay pusher / Galerkin gather on the tile path (mode 0 = push and deposit kernels, mode 5 =
+    the one-kernel particle step; steps after the first sort, drifted particles included) and on the
     per-particle kernel (mode 1); relativistic momenta so
     that the two pushers differ at first order."""
     cfg = small("C2", (24, 16, 16), order=order, dx=(1.0e-6, 0.8e-6, 0.6e-6))
