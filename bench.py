@@ -12,8 +12,11 @@ on BASELINE.json's headline workload, one JSON line on stdout (rank 0).
   (H2D), K steps, pic_get_particles + pic_get_fields (D2H), all inside the timed region.
 * `roofline`= the dominant kernel's algorithmic bytes / flops per launch (DESIGN.md "Byte and flop
   model") over its average launch duration measured by the library's per-kernel CUDA events.
-* `cpu_baseline` = the oracle (oracle/, as it stands, serial) timed on this box's host cores on a
-  bounded sample of the same workload. `--impl reference` times only that.
+* `roofline.peak` = measured: HBM from MEASURED_PEAKS.json, the fp64 pipe and shared-memory bandwidth by
+  the library's own probes (pic_probe_peaks) in this run, before the timed region.
+* `cpu_baseline` = the oracle (oracle/, as it stands) timed on this box's host cores on a bounded sample of
+  the same workload: its OpenMP variant (the paper's CPU scheme; pinned to the serial
+  oracle by T12) on all cores, and the canonical serial oracle on one. `--impl reference` times only that.
 * N>1 (torchrun): the path does not shard: every rank runs
   an independent replica of the workload, no data-path collective; value = N * particles * K / max time.
 """
@@ -38,9 +41,6 @@ import workloads as W  # noqa: E402
 METRIC = "particle-steps/s (sort+gather+push+deposit+Yee)"
 UNIT = "particle-steps/s"
 ATTRS = ("x", "y", "z", "ux", "uy", "uz", "w")
-FP64_FMA_PER_CLK_SM = 64      # measured with the DFMA probe, 64 lanes/clk/SM
-FP32_FMA_PER_CLK_SM = 128
-N_SM = 148
 
 
 # ----------------------------------------------------------------------------- byte / flop model
@@ -176,35 +176,54 @@ def aggregate(n_particles_per_rank, world, steps, ms_max):
 
 
 # ----------------------------------------------------------------------------- the oracle arm
-def time_oracle(cfg_full, steps, warmup, budget_s):
-    """The oracle as it stands (serial, 1 core) on a bounded sample: the same recipe on a smaller box,
-    sized so that warmup+steps oracle steps fit the budget. Returns (value, sample text, ms/step)."""
+def _sample_cfg(cfg_full, n):
+    """The same recipe on an n^3 box (clipped to the configured grid): the bounded sample the oracle is timed on."""
+    shape = tuple(min(n, c) for c in cfg_full.n_cells)
+    if shape == tuple(cfg_full.n_cells):
+        return cfg_full
+    return W.scaled(cfg_full, shape, z_first=0, ramp_cells=0, laser=False)
+
+
+def time_oracle(cfg_full, steps, warmup, budget_s, threads):
+    """The oracle as it stands on a bounded sample of the workload: the largest box of the same recipe whose
+    warmup+steps oracle steps fit the budget (the configured box itself if that fits). threads = 1: the
+    canonical serial oracle; otherwise its OpenMP variant on that many threads (0 = all OpenMP offers).
+    Returns dict(value, sample, ms_per_step, cores, particles)."""
     import oracle
-    t_cal = None
+    cal = _sample_cfg(cfg_full, 16)
+    o = _make_oracle(oracle, cal)
+    used = 1
+    t0 = time.perf_counter()
+    if threads == 1:
+        o.step(1)
+    else:
+        used = o.step_omp(1, threads)
+    t_cal = (time.perf_counter() - t0) / max(cal.n_particles, 1)
+    o.close()
     chosen = None
-    for n in (64, 48, 40, 32, 24, 16, 8):
-        shape = tuple(min(n, c) for c in cfg_full.n_cells)
-        cfg = W.scaled(cfg_full, shape, z_first=0, ramp_cells=0, laser=False)
-        if t_cal is None:
-            # calibrate on the smallest box: seconds per particle-step
-            cal = W.scaled(cfg_full, tuple(min(8, c) for c in cfg_full.n_cells), z_first=0, ramp_cells=0, laser=False)
-            o = _make_oracle(oracle, cal)
-            t0 = time.perf_counter()
-            o.step(1)
-            t_cal = (time.perf_counter() - t0) / max(cal.n_particles, 1)
-            o.close()
-        if cfg.n_particles * t_cal * (steps + warmup) <= budget_s or n == 8:
+    for n in (256, 128, 96, 64, 48, 40, 32, 24, 16, 8):
+        if n > max(cfg_full.n_cells) and n != 8:
+            continue
+        cfg = _sample_cfg(cfg_full, n)
+        # the calibration box is small (threads idle, caches warm): leave a factor of two
+        if cfg.n_particles * t_cal * (steps + warmup) * 2.0 <= budget_s or n == 8:
             chosen = cfg
             break
     o = _make_oracle(oracle, chosen)
-    o.step(warmup)
+    run = (lambda k: o.step(k)) if threads == 1 else (lambda k: o.step_omp(k, threads))
+    if warmup:
+        run(warmup)
     t0 = time.perf_counter()
-    o.step(steps)
+    run(steps)
     dt = time.perf_counter() - t0
     o.close()
-    sample = "%s recipe on a %dx%dx%d box (%d particles), %d oracle steps after %d warm-up" % (
-        cfg_full.name, *chosen.n_cells, chosen.n_particles, steps, warmup)
-    return chosen.n_particles * steps / dt, sample, dt / steps * 1e3
+    whole = tuple(chosen.n_cells) == tuple(cfg_full.n_cells)
+    sample = "%s %s (%d particles), %d oracle steps after %d warm-up, %s" % (
+        cfg_full.name, "at its configured size" if whole else "recipe on a %dx%dx%d box" % tuple(chosen.n_cells),
+        chosen.n_particles, steps, warmup,
+        "serial oracle, 1 thread" if threads == 1 else "OpenMP variant of the oracle, %d threads" % used)
+    return dict(value=chosen.n_particles * steps / dt, sample=sample, ms_per_step=dt / steps * 1e3, cores=used,
+                particles=chosen.n_particles)
 
 
 def _make_oracle(oracle, cfg):
@@ -219,17 +238,24 @@ def _make_oracle(oracle, cfg):
 
 
 def run_reference(args):
+    """The reference arm of this tier is the oracle: its OpenMP variant on all host cores, on a bounded
+    sample of the same workload (the line says which), K steps after W warm-up steps."""
     rank, _, world = dist_env()
     if rank != 0:
         return 0
     cfg = W.CONFIGS[args.config]
-    value, sample, ms = time_oracle(cfg, args.steps, args.warmup, budget_s=150.0)
+    r = time_oracle(cfg, args.steps, args.warmup, budget_s=150.0, threads=0)
+    cd = config_dict(cfg, world, args)
+    cd["timed_sample"] = r["sample"]                 # what this arm ran: a bounded sample of the workload above
+    cd["particles_timed"] = r["particles"]
     line = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": cfg.dtype, "data": "synthetic", "config": config_dict(cfg, world, args),
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
-        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms_per_step"],
+        "ms_per_step_is_for": "%d particles (the timed sample), not the configured %d" % (r["particles"], cfg.n_particles),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": cfg.dtype, "data": "synthetic", "config": cd,
+        "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
+        "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
@@ -301,6 +327,8 @@ def run_ours(args):
         del d
     if E0 is not None:
         sim.set_fields(E0, B0)
+    # on-chip ceilings measured in this run (roofline against measured ceilings)
+    probes = pic.pic_probe_peaks(stream.cuda_stream, 0.0 if args.skip_probe else 0.2)
     sim.step(args.warmup)
     sim.synchronize()
     d0 = sim.diagnostics()
@@ -386,7 +414,7 @@ def run_ours(args):
     if rank != 0:
         return 0
 
-    # ---------------- roofline of the dominant kernel, from the per-kernel device timers
+    # ---------------- rooflines of the particle kernels, from the per-kernel device timers
     m = model(cfg)
     peaks = {}
     try:
@@ -394,64 +422,82 @@ def run_ours(args):
     except Exception:
         pass
     hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
-    hbm_src = "measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)"
+    hbm_src = "hbm: measured (MEASURED_PEAKS.json hbm_gbs)" if "hbm_gbs" in peaks else "hbm: fallback 6650 GB/s (B200_PROFILING.md)"
     clocks = clk.summary()
-    sm_max = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
-    per_clk = FP64_FMA_PER_CLK_SM if cfg.dtype == "f64" else FP32_FMA_PER_CLK_SM
-    alu_peak = N_SM * per_clk * 2 * sm_max * 1e6 / 1e12          # TFLOP/s at the maximum SM clock
+    f64 = cfg.dtype == "f64"
+    # fp64: the DFMA probe for vector kernels, the DMMA probe for the tensor-pipe deposition (same pipe);
+    # fp32: the FFMA probe. Shared memory: the 64-bit load probe.
+    alu_vec = probes["fp64_fma_tflops"] if f64 else probes["fp32_fma_tflops"]
+    alu_mma = probes["fp64_mma_tflops"] if f64 else probes["fp32_fma_tflops"]
+    smem_peak = probes["smem_tbs"]
     per_launch = {k: (v[0] / v[1] if v[1] else 0.0) for k, v in phases.items()}
     n_species = len(cfg.species)
-    dep_name = ("k_deposit_mma (Esirkepov, fp64 tensor pipe)" if cfg.dtype == "f64" and args.deposit_mode in (0, 4)
-                else "k_deposit_tile / k_deposit_coop (Esirkepov, lane groups)")
-    kern = {"push": ("k_push_tile (gather + Boris push)", m["push_bytes"], m["push_flops"]),
-            "deposit": (dep_name, m["deposit_bytes"], m["deposit_flops"])}
-    fused = phases["deposit"][1] == 0
-    if fused:
-        kern = {"push": ("k_particles_global (gather + push + deposit)", m["fused_bytes"],
-                         m["push_flops"] + m["deposit_flops"])}
-    dom = max(kern, key=lambda k: phases[k][0])
-    name, bpp, fpp = kern[dom]
     units = n_part / n_species                      # particles one launch processes
-    dur = per_launch[dom] * 1e-3
-    hbm_ach = bpp * units / dur / 1e9 if dur > 0 else 0.0
-    alu_ach = fpp * units / dur / 1e12 if dur > 0 else 0.0
-    hbm_frac, alu_frac = hbm_ach / hbm_peak, alu_ach / alu_peak
-    if alu_frac >= hbm_frac:
-        roof = {"bound": "alu", "achieved": alu_ach, "peak": alu_peak, "unit": "TFLOP/s", "frac": alu_frac}
+    mode = args.deposit_mode
+    mma = f64 and mode in (0, 4, 5)
+    if phases["deposit"][1] == 0:                   # one kernel does the whole particle step
+        nm = "k_fused_mma (gather + push + deposit, tensor pipe)" if mode == 5 else "k_particles_global (gather + push + deposit)"
+        kern = {"push": (nm, m["fused_bytes"], m["push_flops"] + m["deposit_flops"], alu_mma if mode == 5 else alu_vec,
+                         m["push_smem_bytes"] if mode == 5 else 0)}
     else:
-        roof = {"bound": "hbm", "achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_frac}
-    # dram bytes per launch of that kernel from the committed ncu --set full summary (same workload)
-    traffic, traffic_src = args.traffic, ("--traffic" if args.traffic is not None else None)
-    smem_frac = None            # shared-memory wavefronts / peak from the same ncu capture (the push's real bound)
-    if traffic is None:
-        try:
-            tj = json.load(open(os.path.join(ROOT, "profiles", "traffic_%s.json" % cfg.name)))
-            key = [k for k in tj["dram_bytes_per_launch"] if k in name]
-            if key and args.deposit_mode == 0:
-                traffic, traffic_src = float(tj["dram_bytes_per_launch"][key[0]]), tj["source"]
-                smem_frac = tj.get("shared_wavefront_frac_of_peak", {}).get(key[0])
-        except Exception:
-            pass
+        dep_name = "k_deposit_mma (Esirkepov, fp64 tensor pipe)" if mma else "k_deposit_tile / k_deposit_coop (Esirkepov, lane groups)"
+        kern = {"push": ("k_push_tile (gather + Boris push)", m["push_bytes"], m["push_flops"], alu_vec, m["push_smem_bytes"]),
+                "deposit": (dep_name, m["deposit_bytes"], m["deposit_flops"], alu_mma if mma else alu_vec, 0)}
+    traffic_file = {}
+    try:
+        traffic_file = json.load(open(os.path.join(ROOT, "profiles", "traffic_%s.json" % cfg.name)))
+    except Exception:
+        pass
+    per_kernel = {}
+    for key, (name, bpp, fpp, alu_peak, smem_b) in kern.items():
+        dur = per_launch[key] * 1e-3
+        if dur <= 0:
+            continue
+        e = {"kernel": name, "ms_per_launch": per_launch[key], "launches_timed": phases[key][1],
+             "bytes_per_particle": bpp, "flops_per_particle": fpp,
+             "hbm_gbs": bpp * units / dur / 1e9, "alu_tflops": fpp * units / dur / 1e12, "alu_peak_tflops": alu_peak}
+        e["hbm_frac"] = e["hbm_gbs"] / hbm_peak
+        e["alu_frac"] = e["alu_tflops"] / alu_peak if alu_peak > 0 else None
+        if smem_b:
+            # the roof that actually binds the gather: every stencil value of every
+            # component is one shared-memory read per particle
+            e["smem"] = {"achieved": smem_b * units / dur / 1e12, "peak": smem_peak, "unit": "TB/s",
+                         "frac": (smem_b * units / dur / 1e12) / smem_peak if smem_peak > 0 else None,
+                         "bytes_per_particle": smem_b}
+        tk = [k for k in traffic_file.get("dram_bytes_per_launch", {}) if k in name]
+        if tk and mode == 0:
+            e["traffic"] = float(traffic_file["dram_bytes_per_launch"][tk[0]])
+            e["shared_wavefront_frac_ncu"] = traffic_file.get("shared_wavefront_frac_of_peak", {}).get(tk[0])
+        per_kernel[key] = e
+    dom = max(per_kernel, key=lambda k: per_kernel[k]["ms_per_launch"] * per_kernel[k]["launches_timed"])
+    d = per_kernel[dom]
+    if (d["alu_frac"] or 0) >= d["hbm_frac"]:
+        roof = {"bound": "alu", "achieved": d["alu_tflops"], "peak": d["alu_peak_tflops"], "unit": "TFLOP/s", "frac": d["alu_frac"]}
+    else:
+        roof = {"bound": "hbm", "achieved": d["hbm_gbs"], "peak": hbm_peak, "unit": "GB/s", "frac": d["hbm_frac"]}
+    traffic = args.traffic if args.traffic is not None else d.get("traffic")
     roof.update({
-        "kernel": name, "ms_per_launch": per_launch[dom], "launches_timed": phases[dom][1],
-        "traffic": traffic, "traffic_source": traffic_src, "shared_wavefront_frac_ncu": smem_frac, "hbm_gbs": hbm_ach, "hbm_frac": hbm_frac, "alu_tflops": alu_ach,
-        "alu_frac": alu_frac, "bytes_per_particle": bpp, "flops_per_particle": fpp,
-        "peak_source": hbm_src + "; alu = 148 SM x %d FMA/clk x 2 x %.0f MHz" % (per_clk, sm_max),
+        "kernel": d["kernel"], "ms_per_launch": d["ms_per_launch"], "launches_timed": d["launches_timed"],
+        "traffic": traffic,
+        "traffic_source": "--traffic" if args.traffic is not None else (traffic_file.get("source") if traffic is not None else None),
+        "hbm_gbs": d["hbm_gbs"], "hbm_frac": d["hbm_frac"], "alu_tflops": d["alu_tflops"], "alu_frac": d["alu_frac"],
+        "bytes_per_particle": d["bytes_per_particle"], "flops_per_particle": d["flops_per_particle"],
+        "peak_source": hbm_src + "; alu and shared memory: measured in this run by pic_probe_peaks "
+                       "(%s)" % ("probes skipped" if args.skip_probe else "0.2 s per probe, best launch"),
+        "measured_peaks": probes,
+        "kernels": per_kernel,
         "phase_ms_per_step": {k: v[0] / args.steps for k, v in phases.items()},
     })
-    if dom == "push" and not fused:
-        # the roof that actually binds k_push_tile: shared-memory bandwidth,
-        # 148 SMs x 128 B/clk x SM clock; achieved = algorithmic stencil bytes / launch time
-        smem_peak = N_SM * 128 * sm_max * 1e6 / 1e12
-        smem_ach = m["push_smem_bytes"] * units / dur / 1e12 if dur > 0 else 0.0
-        roof["smem"] = {"achieved": smem_ach, "peak": smem_peak, "unit": "TB/s", "frac": smem_ach / smem_peak,
-                        "bytes_per_particle": m["push_smem_bytes"]}
+    if "smem" in d:
+        roof["smem"] = d["smem"]
     step_gbs = m["step_bytes"] * n_part * args.steps / (ms * 1e-3) / 1e9
 
     cpu = None
     if not args.skip_cpu and world == 1:
-        v, sample, _ = time_oracle(cfg, 4, 0, budget_s=20.0)
-        cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample}
+        par = time_oracle(cfg, 2, 0, budget_s=25.0, threads=0)
+        ser = time_oracle(cfg, 2, 0, budget_s=8.0, threads=1)
+        cpu = {"value": par["value"], "unit": UNIT, "cores": par["cores"], "kind": "oracle", "sample": par["sample"],
+               "serial": {"value": ser["value"], "unit": UNIT, "cores": 1, "sample": ser["sample"]}}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -473,7 +519,7 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=8)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C2", choices=sorted(W.CONFIGS))
-    ap.add_argument("--deposit-mode", type=int, default=0, help="PIC_DEPOSIT_* (0 auto, 1 global, 2 cooperative, 3 tile, 4 tile + fp64 tensor pipe)")
+    ap.add_argument("--deposit-mode", type=int, default=0, help="PIC_DEPOSIT_* (0 auto, 1 global, 2 cooperative, 3 tile, 4 tile + fp64 tensor pipe, 5 one fused kernel)")
     ap.add_argument("--sort-interval", type=int, default=None, help="sweeps: sort every N steps (0 = only never)")
     ap.add_argument("--tile", default=None, help="sweeps: cells per sort bin, e.g. 4,4,4")
     ap.add_argument("--sort-key-mode", type=int, default=0, help="sweeps: 0 cell key inside the tile, 1 tile only")
@@ -483,6 +529,7 @@ def main(argv=None):
     ap.add_argument("--solver", type=int, default=0, help="variants: PIC_SOLVER_* (0 Yee, 1 CKC)")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs: device-resident leg only")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs: do not time the oracle")
+    ap.add_argument("--skip-probe", action="store_true", help="profiling runs: one launch per on-chip probe instead of 0.2 s")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)")
     args = ap.parse_args(argv)

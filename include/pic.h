@@ -119,6 +119,13 @@ typedef struct {
   int32_t pusher;        /* PIC_PUSHER_*; default PIC_PUSHER_BORIS */
   int32_t gather_mode;   /* PIC_GATHER_*; default PIC_GATHER_UNIFORM */
   int32_t solver;        /* PIC_SOLVER_*; default PIC_SOLVER_YEE */
+  int32_t deterministic; /* 0 (default): J is summed with floating-point reductions at L2, in whatever
+                            order the warps arrive, so J differs from run to run in
+                            the last bits. 1: every contribution is split into two 64-bit fixed-point
+                            parts and summed with INTEGER reductions, which are associative: J, and with
+                            it the whole simulation, is bit-identical from run to run (SURVEY.md 8(f)
+                            NEXT-1, "atomic-order-free deposition"). Any deposit_mode. Costs a second
+                            reduction per contribution and 48 bytes per grid node. */
   void*   cuda_stream;   /* cudaStream_t all work is issued on (e.g. torch's current stream);
                             NULL = the legacy default stream */
 } pic_options;
@@ -216,6 +223,24 @@ PIC_API int32_t pic_num_species(const pic_sim* sim);
 /* Text of the last error of this handle ("" if none). sim == NULL: the last pic_create error.
  * The string is owned by the library and valid until the next call on the same handle. */
 PIC_API const char* pic_last_error(const pic_sim* sim);
+
+/* On-chip ceilings of the current CUDA device, measured now: the roofline method of the paper quotes
+ * kernels against MEASURED ceilings (Fig. 2), and the two units that bound the
+ * particle kernels here (the fp64 pipe and shared-memory bandwidth) are in no vendor or driver file.
+ * Each probe (a register-resident loop filling every warp slot of every SM) is launched on `cuda_stream`
+ * (NULL = legacy default) repeatedly for at least `seconds_per_probe` seconds (and at least 3 times); the
+ * best launch is reported. out: host array of PIC_NPROBE doubles. No simulation handle is involved and no
+ * PIC work is done. Synchronises. Errors: INVALID_ARG, CUDA. */
+enum {
+  PIC_PROBE_FP64_FMA_TFLOPS = 0, /* DFMA, 8 independent chains per thread */
+  PIC_PROBE_FP64_MMA_TFLOPS = 1, /* mma.sync.m8n8k4.f64 (the deposit's tensor-pipe instruction), 2 flop per FMA */
+  PIC_PROBE_SMEM_TBS = 2,        /* conflict-free 64-bit shared-memory loads, TB/s */
+  PIC_PROBE_FP32_FMA_TFLOPS = 3, /* FFMA, 16 independent chains per thread */
+  PIC_PROBE_SM_COUNT = 4,        /* multiprocessors of the device */
+  PIC_PROBE_SM_CLOCK_MHZ = 5,    /* the device's nominal maximum SM clock (cudaDevAttrClockRate) */
+  PIC_NPROBE = 6
+};
+PIC_API int pic_probe_peaks(void* cuda_stream, double seconds_per_probe, double* out);
 
 /* The weights the CKC solver (PIC_SOLVER_CKC, ref [12]) uses for cells of size dx[3]: the difference of
  * E along axis a in the B update is alpha[a]*dF(0,0) + beta[3a+b]*[dF(+b) + dF(-b)] + beta[3a+c]*[dF(+c) +

@@ -32,7 +32,7 @@ SYMBOLS = (
     "pic_default_options", "pic_create", "pic_add_species", "pic_set_fields", "pic_step", "pic_synchronize",
     "pic_get_fields", "pic_get_particles", "pic_get_sort_state", "pic_sort_now", "pic_get_diagnostics",
     "pic_get_rho", "pic_enable_phase_timing", "pic_get_phase_times", "pic_num_particles", "pic_num_species",
-    "pic_last_error", "pic_ckc_coefficients", "pic_destroy",
+    "pic_last_error", "pic_ckc_coefficients", "pic_probe_peaks", "pic_destroy",
 )
 
 
@@ -46,7 +46,7 @@ class pic_options(C.Structure):
     _fields_ = [("periodic", C.c_int32 * 3), ("tile", C.c_int32 * 3), ("sort_interval", C.c_int32),
                 ("sort_key_mode", C.c_int32), ("deposit_mode", C.c_int32), ("pusher", C.c_int32),
                 ("gather_mode", C.c_int32), ("solver", C.c_int32),
-                ("cuda_stream", C.c_void_p)]
+                ("deterministic", C.c_int32), ("cuda_stream", C.c_void_p)]
 
 
 _lib = None
@@ -84,6 +84,7 @@ def lib():
         L.pic_last_error.argtypes = [vp]
         L.pic_last_error.restype = C.c_char_p
         L.pic_ckc_coefficients.argtypes = [dp, dp, dp, dp]
+        L.pic_probe_peaks.argtypes = [vp, C.c_double, dp]
         L.pic_destroy.argtypes = [vp]
         L.pic_destroy.restype = None
         _lib = L
@@ -231,6 +232,18 @@ def pic_ckc_coefficients(dx):
     return np.array(al[:]), np.array(be[:]).reshape(3, 3), np.array(ga[:])
 
 
+PROBE_NAMES = ("fp64_fma_tflops", "fp64_mma_tflops", "smem_tbs", "fp32_fma_tflops", "sm_count", "sm_clock_mhz")
+
+
+def pic_probe_peaks(stream=None, seconds_per_probe=0.2) -> dict:
+    """Measured on-chip ceilings of the current device (see include/pic.h)."""
+    out = (C.c_double * len(PROBE_NAMES))()
+    rc = lib().pic_probe_peaks(stream, float(seconds_per_probe), out)
+    if rc != 0:
+        raise PicError(rc, "pic_probe_peaks failed (no CUDA device?)")
+    return dict(zip(PROBE_NAMES, out))
+
+
 def pic_destroy(h):
     lib().pic_destroy(h)
 
@@ -241,7 +254,7 @@ class Sim:
 
     def __init__(self, n_cells, dx, dt, order, dtype=np.float64, periodic=(1, 1, 1), tile=(8, 8, 8),
                  sort_interval=4, sort_key_mode=0, deposit_mode=PIC_DEPOSIT_AUTO, stream=None,
-                 pusher=PIC_PUSHER_BORIS, gather_mode=PIC_GATHER_UNIFORM, solver=PIC_SOLVER_YEE):
+                 pusher=PIC_PUSHER_BORIS, gather_mode=PIC_GATHER_UNIFORM, solver=PIC_SOLVER_YEE, deterministic=False):
         self.dtype = np.dtype(dtype)
         self.n_cells = tuple(int(v) for v in n_cells)
         self.n_valid = self.n_cells[0] * self.n_cells[1] * self.n_cells[2]
@@ -256,6 +269,7 @@ class Sim:
         o.pusher = int(pusher)
         o.gather_mode = int(gather_mode)
         o.solver = int(solver)
+        o.deterministic = 1 if deterministic else 0
         o.cuda_stream = stream
         self._h = pic_create(self.n_cells, dx, dt, order, PIC_F64 if self.dtype == np.float64 else PIC_F32, o)
 

@@ -26,6 +26,12 @@ struct Grid {
   R inv_dx[3], L[3], cB[3], cE[3], cJ, inv_c2, dt;
   R* F[6];           // Ex Ey Ez Bx By Bz
   R* J[3];
+  // deterministic deposition (PIC_DEPOSIT order-free sums): every contribution to J is
+  // split into two 64-bit fixed-point parts that are added with INTEGER reductions (exact, hence independent
+  // of the order in which warps arrive); Jfix[0] / Jfix[1] shadow the three J arrays (same offsets)
+  long long* Jfix[2];
+  double fix_scale[2];   // 2^e_hi, 2^e_lo (e_lo = e_hi + 40); 0 = mode off
+  double fix_inv[2];
   __host__ __device__ __forceinline__ int idx(int i, int j, int k) const { return org + i + sy * j + sz * k; }
   __host__ __device__ __forceinline__ int64_t padded_total() const { return (int64_t)P[0] * P[1] * P[2]; }
 };
@@ -149,5 +155,23 @@ __device__ __forceinline__ int cell_of(R x, R inv_dx, int N) {
 // reduction without return value (RED.E.ADD.F64 / .F32 at L2)
 __device__ __forceinline__ void red_add(double* p, double v) { atomicAdd(p, v); }
 __device__ __forceinline__ void red_add(float* p, float v) { atomicAdd(p, v); }
+
+// One contribution v to the J element at p (p points into g.J[0..2], which are one allocation). Default: a
+// floating-point reduction at L2, whose result depends on the order of arrival. Deterministic mode: v is
+// split into hi = rint(v 2^e_hi) and lo = rint((v - hi 2^-e_hi) 2^e_lo), both added as 64-bit integers;
+// integer addition is associative, so J comes out bit-identical whatever the order (k_fix_to_J converts).
+// 2^e_hi is chosen from a bound no node can exceed (pic_api.cu), the low part carries 40 more bits.
+template <class R>
+__device__ __forceinline__ void j_add(const Grid<R>& g, R* p, R v) {
+  if (g.fix_scale[0] != 0.0) {
+    const long long off = p - g.J[0];
+    const double hi = rint((double)v * g.fix_scale[0]);
+    const double lo = rint(((double)v - hi * g.fix_inv[0]) * g.fix_scale[1]);
+    atomicAdd(reinterpret_cast<unsigned long long*>(g.Jfix[0] + off), (unsigned long long)(long long)hi);
+    atomicAdd(reinterpret_cast<unsigned long long*>(g.Jfix[1] + off), (unsigned long long)(long long)lo);
+  } else {
+    red_add(p, v);
+  }
+}
 
 }  // namespace pic

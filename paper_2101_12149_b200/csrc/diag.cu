@@ -1,5 +1,7 @@
 // Input validation and diagnostics reductions (support, not on the hot path; PAPER.md:98-102
 // §2.6: several reductions in one launch). All accumulators are fp64.
+#include <algorithm>
+
 #include "internal.h"
 
 namespace pic {
@@ -160,6 +162,24 @@ void launch_validate_array(const R* a, int64_t n, int* flags, Ctx& c) {
   k_validate_array<R><<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(a, n, flags);
   c.launches++;
 }
+// max |a| into *out (non-negative doubles order like their bit patterns, so an integer atomicMax does it
+// exactly and independently of the order of arrival)
+template <class R>
+__global__ void __launch_bounds__(256) k_max_abs(const R* __restrict__ a, int64_t n, double* out) {
+  double m = 0.0;
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (int64_t)gridDim.x * blockDim.x)
+    m = fmax(m, fabs((double)a[t]));
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+  if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<unsigned long long*>(out), (unsigned long long)__double_as_longlong(m));
+}
+template <class R>
+void launch_max_abs(const R* a, int64_t n, double* out1, Ctx& c) {
+  if (n == 0) return;
+  const int64_t nb = std::min<int64_t>((n + 255) / 256, (int64_t)c.sm_count * 16);
+  k_max_abs<R><<<(unsigned)nb, 256, 0, c.stream>>>(a, n, out1);
+  c.launches++;
+}
 template <class R>
 void launch_field_energy(const Grid<R>& g, double* out2, Ctx& c) {
   k_field_energy<R><<<grd(g.N[0], g.N[1], g.N[2]), blk(), 0, c.stream>>>(g, out2);
@@ -189,6 +209,7 @@ void launch_gauss(const Grid<R>& g, const double* rho, double* out2, Ctx& c) {
 #define INST(R)                                                                                    \
   template void launch_validate_particles<R>(const Grid<R>&, const Particles<R>&, int*, Ctx&);     \
   template void launch_validate_array<R>(const R*, int64_t, int*, Ctx&);                           \
+  template void launch_max_abs<R>(const R*, int64_t, double*, Ctx&);                               \
   template void launch_field_energy<R>(const Grid<R>&, double*, Ctx&);                             \
   template void launch_particle_sums<R>(const Particles<R>&, double, double, double*, Ctx&);       \
   template void launch_rho<R>(const Grid<R>&, const Particles<R>&, int, double, double*, Ctx&);    \

@@ -200,6 +200,19 @@ void launch_push_E(const Grid<R>& g, const int lo[3], const int hi[3], Ctx& c) {
   k_push_E<R><<<grd(b.n[0], b.n[1], b.n[2]), blk(), 0, c.stream>>>(g, b);
   c.launches++;
 }
+// deterministic deposition: the two fixed-point parts of every J element -> J (common.cuh, j_add)
+template <class R>
+__global__ void __launch_bounds__(256) k_fix_to_J(Grid<R> g, int64_t n) {
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  g.J[0][t] = (R)((double)g.Jfix[0][t] * g.fix_inv[0] + (double)g.Jfix[1][t] * g.fix_inv[1]);
+}
+template <class R>
+void launch_fix_to_J(const Grid<R>& g, Ctx& c) {
+  const int64_t n = 3 * g.padded_total();   // the three J arrays are one allocation
+  k_fix_to_J<R><<<(unsigned)((n + 255) / 256), 256, 0, c.stream>>>(g, n);
+  c.launches++;
+}
 template <class R>
 void launch_fold_J(const Grid<R>& g, Ctx& c) {
   if (g.N[0] >= 2 * kGuard && g.N[1] >= 2 * kGuard && g.N[2] >= 2 * kGuard) {
@@ -234,6 +247,7 @@ void launch_unpack(const Grid<R>& g, const R* src, R* dst, Ctx& c) {
   template void launch_push_B<R>(const Grid<R>&, const int*, const int*, Ctx&);         \
   template void launch_push_E<R>(const Grid<R>&, const int*, const int*, Ctx&);         \
   template void launch_fold_J<R>(const Grid<R>&, Ctx&);                                 \
+  template void launch_fix_to_J<R>(const Grid<R>&, Ctx&);                               \
   template void launch_fill_guards<R>(const Grid<R>&, R* const*, int, Ctx&);            \
   template void launch_pack<R>(const Grid<R>&, const R*, R*, Ctx&);                     \
   template void launch_unpack<R>(const Grid<R>&, const R*, R*, Ctx&);

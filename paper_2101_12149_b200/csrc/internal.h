@@ -97,6 +97,7 @@ enum { kPhaseSort = 0, kPhasePush = 1, kPhaseDeposit = 2, kPhaseStray = 3, kPhas
 template <class R> void launch_push_B(const Grid<R>& g, const int lo[3], const int hi[3], Ctx& c);
 template <class R> void launch_push_E(const Grid<R>& g, const int lo[3], const int hi[3], Ctx& c);
 template <class R> void launch_fold_J(const Grid<R>& g, Ctx& c);
+template <class R> void launch_fix_to_J(const Grid<R>& g, Ctx& c);   // deterministic deposition: fixed point -> J
 template <class R> void launch_fill_guards(const Grid<R>& g, R* const* arrays, int narr, Ctx& c);
 template <class R> void launch_pack(const Grid<R>& g, const R* valid_src, R* padded_dst, Ctx& c);
 template <class R> void launch_unpack(const Grid<R>& g, const R* padded_src, R* valid_dst, Ctx& c);
@@ -161,6 +162,8 @@ template <class R>
 void launch_field_energy(const Grid<R>& g, double* out2, Ctx& c);              // out2[0]=sum E^2, [1]=sum B^2
 template <class R>
 void launch_particle_sums(const Particles<R>& p, double q, double m, double* out2, Ctx& c);  // KE, charge
+template <class R>
+void launch_max_abs(const R* a, int64_t n, double* out1, Ctx& c);   // *out1 = max(*out1, max |a|), out1 >= 0
 template <class R>
 void launch_rho(const Grid<R>& g, const Particles<R>& p, int order, double q, double* rho, Ctx& c);
 template <class R>

@@ -233,7 +233,7 @@ __device__ __forceinline__ void deposit_global(const Grid<R>& g, const R* jf, R 
       for (int i = 0; i < NW - 1; ++i) {
         pre += DS[0][i] * c;
         R v = fx * pre;
-        if (v != R(0)) red_add(Jx + base + i + sy * j + sz * k, v);
+        if (v != R(0)) j_add<R>(g, Jx + base + i + sy * j + sz * k, v);
       }
     }
 #pragma unroll
@@ -246,7 +246,7 @@ __device__ __forceinline__ void deposit_global(const Grid<R>& g, const R* jf, R 
       for (int j = 0; j < NW - 1; ++j) {
         pre += DS[1][j] * c;
         R v = fy * pre;
-        if (v != R(0)) red_add(Jy + base + i + sy * j + sz * k, v);
+        if (v != R(0)) j_add<R>(g, Jy + base + i + sy * j + sz * k, v);
       }
     }
 #pragma unroll
@@ -259,7 +259,7 @@ __device__ __forceinline__ void deposit_global(const Grid<R>& g, const R* jf, R 
       for (int k = 0; k < NW - 1; ++k) {
         pre += DS[2][k] * c;
         R v = fz * pre;
-        if (v != R(0)) red_add(Jz + base + i + sy * j + sz * k, v);
+        if (v != R(0)) j_add<R>(g, Jz + base + i + sy * j + sz * k, v);
       }
     }
 }

@@ -137,9 +137,9 @@ __global__ void __launch_bounds__(kCoopWarps * 32) k_deposit_coop(Grid<R> g, Par
     R* jz = g.J[2] + cur_ib + off_jk;
 #pragma unroll
     for (int i = 0; i < NW; ++i) {
-      if (i < NW - 1 && ax[i] != R(0)) red_add(jx + i, ax[i]);
-      if (ay[i] != R(0)) red_add(jy + i, ay[i]);
-      if (az[i] != R(0)) red_add(jz + i, az[i]);
+      if (i < NW - 1 && ax[i] != R(0)) j_add<R>(g, jx + i, ax[i]);
+      if (ay[i] != R(0)) j_add<R>(g, jy + i, ay[i]);
+      if (az[i] != R(0)) j_add<R>(g, jz + i, az[i]);
     }
   };
   auto zero_all = [&]() {
@@ -148,9 +148,9 @@ __global__ void __launch_bounds__(kCoopWarps * 32) k_deposit_coop(Grid<R> g, Par
   };
   auto shift_one = [&]() {   // the run moves one cell up in x: x-slot 0 is complete
     if (lane_on) {
-      if (ax[0] != R(0)) red_add(g.J[0] + cur_ib + off_jk, ax[0]);
-      if (ay[0] != R(0)) red_add(g.J[1] + cur_ib + off_jk, ay[0]);
-      if (az[0] != R(0)) red_add(g.J[2] + cur_ib + off_jk, az[0]);
+      if (ax[0] != R(0)) j_add<R>(g, g.J[0] + cur_ib + off_jk, ax[0]);
+      if (ay[0] != R(0)) j_add<R>(g, g.J[1] + cur_ib + off_jk, ay[0]);
+      if (az[0] != R(0)) j_add<R>(g, g.J[2] + cur_ib + off_jk, az[0]);
     }
 #pragma unroll
     for (int i = 0; i < NW - 1; ++i) { ay[i] = ay[i + 1]; az[i] = az[i + 1]; if (i < NW - 2) ax[i] = ax[i + 1]; }
@@ -331,7 +331,7 @@ __global__ void __launch_bounds__(128) k_deposit_list_warp(Grid<R> g, Particles<
         const R S0b = s_ax[warp][b][0][sl[b]], DSb = s_ax[warp][b][1][sl[b]];
         const R c = S0a * S0b + half * DSa * S0b + half * S0a * DSb + third * DSa * DSb;
         const R v = f * (s_ax[warp][d][2][sl[d]] * c);
-        if (v != R(0)) red_add(g.J[d] + base + i + g.sy * j + g.sz * k, v);
+        if (v != R(0)) j_add<R>(g, g.J[d] + base + i + g.sy * j + g.sz * k, v);
       }
     }
     if (lane == 0) {

@@ -89,6 +89,8 @@ struct Sim : SimBase {
   int order = 1;
   int sort_interval = 4;
   int deposit_mode = 0;
+  bool deterministic = false;   // pic_options.deterministic: J by integer reductions (common.cuh, j_add)
+  double j_bound = 0;           // no J element can exceed this in magnitude (sum over species of n max|w| |q| / (dt dA))
   double dx[3]{}, dt = 0;
   Ctx ctx;
   Pool pool;
@@ -134,6 +136,7 @@ struct Sim : SimBase {
     dt = dt_;
     sort_interval = o.sort_interval;
     deposit_mode = o.deposit_mode;
+    deterministic = o.deterministic != 0;
     ctx.stream = (cudaStream_t)o.cuda_stream;
     PIC_CUDA(cudaGetDevice(&ctx.device));
     PIC_CUDA(cudaDeviceGetAttribute(&ctx.sm_count, cudaDevAttrMultiProcessorCount, ctx.device));
@@ -181,6 +184,14 @@ struct Sim : SimBase {
     for (int c = 0; c < 6; ++c) g.F[c] = base + (size_t)tot * c;
     for (int c = 0; c < 3; ++c) g.J[c] = base + (size_t)tot * (6 + c);
     PIC_CUDA(cudaMemsetAsync(base, 0, (size_t)tot * 9 * sizeof(R), ctx.stream));
+    g.Jfix[0] = g.Jfix[1] = nullptr;
+    g.fix_scale[0] = g.fix_scale[1] = g.fix_inv[0] = g.fix_inv[1] = 0.0;
+    if (deterministic) {
+      long long* fx = palloc<long long>((size_t)tot * 6);
+      if (!fx) return fail(PIC_ERR_OOM, "fixed-point J allocation failed");
+      g.Jfix[0] = fx;
+      g.Jfix[1] = fx + (size_t)tot * 3;
+    }
     d_deact = palloc<unsigned long long>(1);
     d_flags = palloc<int>(2);
     d_red = palloc<double>(8);
@@ -291,6 +302,26 @@ struct Sim : SimBase {
     if (f[1]) { cleanup(); return fail(PIC_ERR_OUT_OF_DOMAIN, "particle position outside [0, L)"); }
     rc = ensure_scratch(n);
     if (rc) { cleanup(); return rc; }
+    if (deterministic && n > 0) {
+      // every contribution of a particle to a J element is at most |q| w / (dt dA) in magnitude (the prefix of
+      // the Esirkepov weights is a difference of shape products), so n max|w| |q| / (dt min dA) bounds any sum;
+      // max is exact and order-free, so the scale below is the same in every run
+      double wmax = 0.0;
+      cudaMemsetAsync(d_red, 0, sizeof(double), ctx.stream);
+      launch_max_abs<R>(p.w, n, d_red, ctx);
+      PIC_CUDA(cudaMemcpyAsync(&wmax, d_red, sizeof(double), cudaMemcpyDeviceToHost, ctx.stream));
+      PIC_CUDA(cudaStreamSynchronize(ctx.stream));
+      const double dA = std::min(dx[0] * dx[1], std::min(dx[1] * dx[2], dx[0] * dx[2]));
+      j_bound += (double)n * wmax * std::fabs(q) / (dt * dA);
+      if (j_bound > 0) {
+        int e = 0;
+        std::frexp(j_bound, &e);                       // j_bound < 2^e
+        g.fix_scale[0] = std::ldexp(1.0, 61 - e);      // |sum| 2^(61-e) < 2^61: no overflow, whatever arrives
+        g.fix_scale[1] = std::ldexp(1.0, 61 - e + 40); // the low part: 40 more bits, |lo| <= 2^39 per contribution
+        g.fix_inv[0] = 1.0 / g.fix_scale[0];
+        g.fix_inv[1] = 1.0 / g.fix_scale[1];
+      }
+    }
     species.push_back(sp);
     if (id) *id = (int32_t)species.size() - 1;
     return PIC_OK;
@@ -403,10 +434,12 @@ struct Sim : SimBase {
       {
         ScopedPhase ph(ctx, kPhaseFields);
         cudaMemsetAsync(g.J[0], 0, jbytes, ctx.stream);   // the three J arrays are contiguous
+        if (deterministic) cudaMemsetAsync(g.Jfix[0], 0, (size_t)g.padded_total() * 6 * sizeof(long long), ctx.stream);
       }
       for (auto& sp : species) particle_step(sp);         // timed per kernel in particles.cu
       {
         ScopedPhase ph(ctx, kPhaseFields);
+        if (deterministic && g.fix_scale[0] != 0.0) launch_fix_to_J<R>(g, ctx);   // integer sums -> J
         launch_fold_J<R>(g, ctx);                    // SumBoundary
         launch_fill_guards<R>(g, g.J, 3, ctx);       // J images for the widened E update
         launch_push_B<R>(g, loB, hiB, ctx);          // widened by one layer on periodic axes, so
@@ -589,6 +622,7 @@ void pic_default_options(pic_options* o) {
   o->pusher = PIC_PUSHER_BORIS;
   o->gather_mode = PIC_GATHER_UNIFORM;
   o->solver = PIC_SOLVER_YEE;
+  o->deterministic = 0;
   o->cuda_stream = nullptr;
 }
 
@@ -606,7 +640,7 @@ int pic_create(const int32_t n_cells[3], const double dx[3], double dt, int shap
   if (prec != PIC_F64 && prec != PIC_F32) return bad(PIC_ERR_INVALID_ARG, "unknown precision");
   if (o.sort_interval < 0 || o.sort_key_mode < 0 || o.sort_key_mode > 1 || o.deposit_mode < 0 ||
       o.deposit_mode > 5 || o.pusher < 0 || o.pusher > 1 || o.gather_mode < 0 || o.gather_mode > 1 ||
-      o.solver < 0 || o.solver > 1)
+      o.solver < 0 || o.solver > 1 || o.deterministic < 0 || o.deterministic > 1)
     return bad(PIC_ERR_INVALID_ARG, "bad option value");
   double s2 = 0;
   for (int d = 0; d < 3; ++d) {

@@ -322,20 +322,20 @@ __device__ __forceinline__ R group_sum(R v) {
 // one physical slot (static P), summed over the groups -> the J element jx points at, then cleared.
 // Warp-uniform.
 template <class R, int ORDER, int P>
-__device__ __forceinline__ void flush_slot(Acc<R, TWin<ORDER>::NX>& a, const JPtr<R>& jx, bool writer) {
+__device__ __forceinline__ void flush_slot(const Grid<R>& g, Acc<R, TWin<ORDER>::NX>& a, const JPtr<R>& jx, bool writer) {
   using W = TWin<ORDER>;
   const R vx = group_sum<R, W::LG>(a.x[P]), vy = group_sum<R, W::LG>(a.y[P]), vz = group_sum<R, W::LG>(a.z[P]);
   if (writer) {
-    if (vx != R(0)) red_add(jx.p[0], vx);
-    if (vy != R(0)) red_add(jx.p[1], vy);
-    if (vz != R(0)) red_add(jx.p[2], vz);
+    if (vx != R(0)) j_add<R>(g, jx.p[0], vx);
+    if (vy != R(0)) j_add<R>(g, jx.p[1], vy);
+    if (vz != R(0)) j_add<R>(g, jx.p[2], vz);
   }
   a.x[P] = 0; a.y[P] = 0; a.z[P] = 0;
 }
 
 // all slots: physical slot p holds logical slot (p - ph) mod NX of the window at jx. Warp-uniform.
 template <class R, int ORDER>
-__device__ __forceinline__ void flush_window(Acc<R, TWin<ORDER>::NX>& a, const JPtr<R>& jx, int ph, bool writer) {
+__device__ __forceinline__ void flush_window(const Grid<R>& g, Acc<R, TWin<ORDER>::NX>& a, const JPtr<R>& jx, int ph, bool writer) {
   using W = TWin<ORDER>;
   constexpr int NX = W::NX;
 #pragma unroll
@@ -344,9 +344,9 @@ __device__ __forceinline__ void flush_window(Acc<R, TWin<ORDER>::NX>& a, const J
     i += i < 0 ? NX : 0;
     const R vx = group_sum<R, W::LG>(a.x[p]), vy = group_sum<R, W::LG>(a.y[p]), vz = group_sum<R, W::LG>(a.z[p]);
     if (writer) {
-      if (vx != R(0)) red_add(jx.p[0] + i, vx);
-      if (vy != R(0)) red_add(jx.p[1] + i, vy);
-      if (vz != R(0)) red_add(jx.p[2] + i, vz);
+      if (vx != R(0)) j_add<R>(g, jx.p[0] + i, vx);
+      if (vy != R(0)) j_add<R>(g, jx.p[1] + i, vy);
+      if (vz != R(0)) j_add<R>(g, jx.p[2] + i, vz);
     }
   }
   a.zero();
@@ -355,12 +355,12 @@ __device__ __forceinline__ void flush_window(Acc<R, TWin<ORDER>::NX>& a, const J
 // the particles of one cell (cnt of them, record slots listed in order[]): NG at a time, one per
 // group. PH = (first box node of the cell's window) mod NX; adv = the window moved up one cell.
 template <class R, int ORDER, int PH>
-__device__ __forceinline__ void cell_batch(Acc<R, TWin<ORDER>::NX>& a, bool adv, const JPtr<R>& jx_old, bool writer,
+__device__ __forceinline__ void cell_batch(const Grid<R>& g, Acc<R, TWin<ORDER>::NX>& a, bool adv, const JPtr<R>& jx_old, bool writer,
                                            const R* __restrict__ rec, const int* __restrict__ order, int cnt, int grp,
                                            int j, int k) {
   using W = TWin<ORDER>;
   constexpr int NX = W::NX, NG = 32 / W::LG;
-  if (adv) flush_slot<R, ORDER, (PH + NX - 1) % NX>(a, jx_old, writer);
+  if (adv) flush_slot<R, ORDER, (PH + NX - 1) % NX>(g, a, jx_old, writer);
 #pragma unroll 1
   for (int it = grp; it < cnt; it += NG) accumulate<R, ORDER, PH>(a, rec + order[it] * W::REC, j, k);
 }
@@ -465,15 +465,15 @@ __global__ void __launch_bounds__(NWARP * 32, 2)
       const bool adv = ib == cur + 1;
       JPtr<R> jx_old{};
       if (cur != INT_MIN) jx_old = column(cur);
-      if (ib != cur && !adv && cur != INT_MIN) flush_window<R, ORDER>(acc, jx_old, curph, grp == 0);
+      if (ib != cur && !adv && cur != INT_MIN) flush_window<R, ORDER>(g, acc, jx_old, curph, grp == 0);
       const int* ord = s_order[warp];
       switch (ph) {
-        case 0: cell_batch<R, ORDER, 0>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 1: cell_batch<R, ORDER, 1>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 2: cell_batch<R, ORDER, 2>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 3: cell_batch<R, ORDER, 3 % NX>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 4: cell_batch<R, ORDER, 4 % NX>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        default: cell_batch<R, ORDER, 5 % NX>(acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 0: cell_batch<R, ORDER, 0>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 1: cell_batch<R, ORDER, 1>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 2: cell_batch<R, ORDER, 2>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 3: cell_batch<R, ORDER, 3 % NX>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 4: cell_batch<R, ORDER, 4 % NX>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        default: cell_batch<R, ORDER, 5 % NX>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
       }
       cur = ib;
       curph = ph;
@@ -499,7 +499,7 @@ __global__ void __launch_bounds__(NWARP * 32, 2)
       xn[t] = x1[0]; yn[t] = x1[1]; zn[t] = x1[2];
     }
   }
-  if (cur != INT_MIN) flush_window<R, ORDER>(acc, column(cur), curph, grp == 0);
+  if (cur != INT_MIN) flush_window<R, ORDER>(g, acc, column(cur), curph, grp == 0);
 }
 
 // =================================================================== Esirkepov on the fp64 tensor pipe
@@ -602,9 +602,9 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
           if (cok[b][c]) {
-            if (C.x[b][c] != 0.0) red_add(g.J[0] + base + coff[b][c], (R)C.x[b][c]);
-            if (C.y[b][c] != 0.0) red_add(g.J[1] + base + coff[b][c], (R)C.y[b][c]);
-            if (C.z[b][c] != 0.0) red_add(g.J[2] + base + coff[b][c], (R)C.z[b][c]);
+            if (C.x[b][c] != 0.0) j_add<R>(g, g.J[0] + base + coff[b][c], (R)C.x[b][c]);
+            if (C.y[b][c] != 0.0) j_add<R>(g, g.J[1] + base + coff[b][c], (R)C.y[b][c]);
+            if (C.z[b][c] != 0.0) j_add<R>(g, g.J[2] + base + coff[b][c], (R)C.z[b][c]);
           }
           C.x[b][c] = 0; C.y[b][c] = 0; C.z[b][c] = 0;
         }
@@ -835,9 +835,9 @@ __global__ void __launch_bounds__(NWARP * 32, 1)
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
           if (cok[b][c]) {
-            if (C.x[b][c] != 0.0) red_add(g.J[0] + base + coff[b][c], C.x[b][c]);
-            if (C.y[b][c] != 0.0) red_add(g.J[1] + base + coff[b][c], C.y[b][c]);
-            if (C.z[b][c] != 0.0) red_add(g.J[2] + base + coff[b][c], C.z[b][c]);
+            if (C.x[b][c] != 0.0) j_add<R>(g, g.J[0] + base + coff[b][c], C.x[b][c]);
+            if (C.y[b][c] != 0.0) j_add<R>(g, g.J[1] + base + coff[b][c], C.y[b][c]);
+            if (C.z[b][c] != 0.0) j_add<R>(g, g.J[2] + base + coff[b][c], C.z[b][c]);
           }
           C.x[b][c] = 0; C.y[b][c] = 0; C.z[b][c] = 0;
         }

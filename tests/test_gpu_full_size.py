@@ -233,3 +233,22 @@ def test_C5_full_size_two_species_through_the_resort():
     assert abs(d["charge"] - d0["charge"]) < 1e-12 * qtot
     assert abs(d["gauss_max"] - d0["gauss_max"]) < 1e-9 * d0["rho_max"]
     assert d["deactivated"] == 0
+
+
+def test_C2_full_size_deterministic_deposition_twice():
+    """SURVEY.md 8(f) NEXT-1 at the bench workload's size: with pic_options.deterministic two runs of C2 give
+    bit-identical J, E, B after 5 steps (tile kernels on 4096 CTAs, the stray pass, a re-sort), and the same
+    physics as the default floating-point reductions to roundoff."""
+    cfg = W.CONFIGS["C2"]
+    out = []
+    for det in (True, True, False):
+        _, g, _ = make_pair(cfg, with_oracle=False, gpu_kwargs=dict(deterministic=det))
+        g.step(5)
+        out.append(g.get_fields())
+        del g
+    for grp in range(3):
+        for a, b in zip(out[0][grp], out[1][grp]):
+            assert np.array_equal(a, b)
+    jscale = max(np.max(np.abs(a)) for a in out[0][2])
+    for a, b in zip(out[0][2], out[2][2]):
+        assert np.max(np.abs(a - b)) <= 1e-12 * jscale

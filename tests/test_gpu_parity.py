@@ -506,3 +506,52 @@ def test_full_size_sampled_parity_and_invariants(name, tol):
     assert d["charge"] == pytest.approx(d0["charge"], rel=1e-12)
     assert abs(d["gauss_max"] - d0["gauss_max"]) < (1e-9 if tol == TOL64 else 1e-3) * d0["rho_max"]
     assert d["deactivated"] == 0
+
+
+# ------------------------------------------------------------------ order-free deposition
+@pytest.mark.parametrize("mode", [0, 1, 3, 5])
+def test_deterministic_deposition_is_bit_identical_run_to_run(mode):
+    """pic_options.deterministic: J is summed with integer reductions (two fixed-point parts per contribution),
+    which are associative, so two runs of the same inputs agree BIT FOR BIT in every array after many steps —
+    hot plasma, stale order, the per-particle (stray) pass and a re-sort included — and still match the oracle.
+    PAPER.md:169-175 (the deposit race), SURVEY.md 8(f) NEXT-1."""
+    cfg = small("C2", (24, 16, 16), order=3, dx=(1.0e-6, 0.8e-6, 0.6e-6))
+    cfg.species[0].sigma = 0.3
+    runs = []
+    o = None
+    for rep in range(2):
+        oo, g, _ = make_pair(cfg, fields="random", gpu_kwargs=dict(deposit_mode=mode, deterministic=True),
+                             with_oracle=(rep == 0))
+        o = oo or o
+        g.step(1)
+        if rep == 0:
+            o.step(1)
+            errs = compare_state(o, g, TOL64)
+            assert errs["J"] <= 2e-14, errs            # nothing but the fp64 rounding of each contribution is left
+        g.step(5)
+        runs.append((g.get_fields(), g.get_particles(0)))
+    for grp in range(3):
+        for a, b in zip(runs[0][0][grp], runs[1][0][grp]):
+            assert np.array_equal(a, b)
+    for k in ("id", "x", "y", "z", "ux", "uy", "uz", "w"):
+        assert np.array_equal(runs[0][1][k], runs[1][1][k]), k
+    o.step(5)
+    compare_state(o, g, 50 * TOL64)
+
+
+def test_deterministic_deposition_fp32_and_two_species():
+    """The same in fp32 (the fixed-point parts are formed from the float contribution in double) with two
+    species, whose bounds add up in the fixed-point scale."""
+    cfg = small("C5", (16, 16, 16), dtype="f32", order=2)
+    runs = []
+    for rep in range(2):
+        o, g, _ = make_pair(cfg, fields="random", gpu_kwargs=dict(deterministic=True), with_oracle=(rep == 0))
+        g.step(1)
+        if rep == 0:
+            o.step(1)
+            compare_state(o, g, TOL32, n_species=2)
+        g.step(4)
+        runs.append(g.get_fields())
+    for grp in range(3):
+        for a, b in zip(runs[0][grp], runs[1][grp]):
+            assert np.array_equal(a, b)
