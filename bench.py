@@ -273,7 +273,8 @@ def config_dict(cfg, world, args):
         "l2": "inputs larger than L2 (particle state %.2f GB per buffer vs 126 MB L2)" % (
             cfg.n_particles * (7 * (8 if cfg.dtype == "f64" else 4) + 8) / 1e9),
         "deposit_mode": args.deposit_mode,
-        "variant": {"pusher": args.pusher, "gather_mode": args.gather_mode, "solver": args.solver},
+        "variant": {"pusher": args.pusher, "gather_mode": args.gather_mode, "solver": args.solver,
+                    "deterministic": bool(args.deterministic), "cuda_graph": not args.no_graph},
     }
 
 
@@ -317,7 +318,7 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     kw = dict(dtype=np_dt, periodic=cfg.periodic, tile=cfg.tile, sort_interval=cfg.sort_interval,
               deposit_mode=args.deposit_mode, sort_key_mode=args.sort_key_mode, stream=stream.cuda_stream,
-              pusher=args.pusher, gather_mode=args.gather_mode, solver=args.solver)
+              pusher=args.pusher, gather_mode=args.gather_mode, solver=args.solver, deterministic=args.deterministic, cuda_graph=not args.no_graph)
 
     # ---------------- leg 1: state resident in HBM
     sim = pic.Sim(cfg.n_cells, cfg.dx, cfg.dt, cfg.order, **kw)
@@ -332,8 +333,6 @@ def run_ours(args):
     sim.step(args.warmup)
     sim.synchronize()
     d0 = sim.diagnostics()
-    sim.enable_phase_timing(True)
-    sim.phase_times(reset=True)
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier(dist)
     torch.cuda.synchronize()
@@ -344,9 +343,15 @@ def run_ours(args):
         torch.cuda.synchronize()
     barrier(dist)
     ms = ev0.elapsed_time(ev1)
+    d1 = sim.diagnostics()
+    # per-kernel device times: the same K steps again with the library's CUDA-event timers on (one span per
+    # launch; this pass launches kernel by kernel, the timed region above replays captured graphs)
+    sim.enable_phase_timing(True)
+    sim.phase_times(reset=True)
+    sim.step(args.steps)
+    sim.synchronize()
     phases = sim.phase_times(reset=True)
     sim.enable_phase_timing(False)
-    d1 = sim.diagnostics()
     launches = int(d1["step_launches"] - d0["step_launches"])
     ms_max = max_over_ranks(dist, ms, dev)
     value = aggregate(n_part, world, args.steps, ms_max)
@@ -527,6 +532,8 @@ def main(argv=None):
     ap.add_argument("--pusher", type=int, default=0, help="variants: PIC_PUSHER_* (0 Boris, 1 Vay)")
     ap.add_argument("--gather-mode", type=int, default=0, help="variants: PIC_GATHER_* (0 uniform, 1 Galerkin)")
     ap.add_argument("--solver", type=int, default=0, help="variants: PIC_SOLVER_* (0 Yee, 1 CKC)")
+    ap.add_argument("--deterministic", action="store_true", help="variants: pic_options.deterministic (integer reductions into J)")
+    ap.add_argument("--no-graph", action="store_true", help="variants: launch every kernel of a step separately (pic_options.cuda_graph = 0)")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs: device-resident leg only")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs: do not time the oracle")
     ap.add_argument("--skip-probe", action="store_true", help="profiling runs: one launch per on-chip probe instead of 0.2 s")

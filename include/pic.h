@@ -126,6 +126,11 @@ typedef struct {
                             it the whole simulation, is bit-identical from run to run (SURVEY.md 8(f)
                             NEXT-1, "atomic-order-free deposition"). Any deposit_mode. Costs a second
                             reduction per contribution and 48 bytes per grid node. */
+  int32_t cuda_graph;    /* 1 (default): pic_step captures each time step once per buffer arrangement
+                            (they repeat with period 2 x sort_interval) and replays it as ONE graph launch
+                            (launch latency dominates once the kernels are fast). The first
+                            step of a handle, and every step while phase timing is on, is launched kernel
+                            by kernel. 0: always kernel by kernel. Results are identical either way. */
   void*   cuda_stream;   /* cudaStream_t all work is issued on (e.g. torch's current stream);
                             NULL = the legacy default stream */
 } pic_options;

@@ -161,9 +161,11 @@ __device__ __forceinline__ void red_add(float* p, float v) { atomicAdd(p, v); }
 // split into hi = rint(v 2^e_hi) and lo = rint((v - hi 2^-e_hi) 2^e_lo), both added as 64-bit integers;
 // integer addition is associative, so J comes out bit-identical whatever the order (k_fix_to_J converts).
 // 2^e_hi is chosen from a bound no node can exceed (pic_api.cu), the low part carries 40 more bits.
-template <class R>
+// DET: 0 = floating-point reduction, 1 = fixed point, -1 = whichever the grid says (run-time test; the hot
+// kernels are compiled for both and never pay for it).
+template <class R, int DET = -1>
 __device__ __forceinline__ void j_add(const Grid<R>& g, R* p, R v) {
-  if (g.fix_scale[0] != 0.0) {
+  if (DET == 1 || (DET == -1 && g.fix_scale[0] != 0.0)) {
     const long long off = p - g.J[0];
     const double hi = rint((double)v * g.fix_scale[0]);
     const double lo = rint(((double)v - hi * g.fix_inv[0]) * g.fix_scale[1]);

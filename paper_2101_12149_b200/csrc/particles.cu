@@ -284,7 +284,7 @@ __global__ void __launch_bounds__(128) k_deposit_list(Grid<R> g, Particles<R> p,
 // window of ORDER+2 nodes: S0, DS, running sum of DS) in shared memory, then the 32 lanes walk the
 // particle's nodes with x fastest, so that one RED instruction covers runs of 4-5 contiguous elements
 // instead of 32 unrelated ones (L2 reduction throughput is about 2x better for contiguous lanes).
-template <class R, int ORDER>
+template <class R, int ORDER, int DET>
 __global__ void __launch_bounds__(128) k_deposit_list_warp(Grid<R> g, Particles<R> p, R* __restrict__ xn,
                                                            R* __restrict__ yn, R* __restrict__ zn,
                                                            const int32_t* __restrict__ list,
@@ -331,7 +331,7 @@ __global__ void __launch_bounds__(128) k_deposit_list_warp(Grid<R> g, Particles<
         const R S0b = s_ax[warp][b][0][sl[b]], DSb = s_ax[warp][b][1][sl[b]];
         const R c = S0a * S0b + half * DSa * S0b + half * S0a * DSb + third * DSa * DSb;
         const R v = f * (s_ax[warp][d][2][sl[d]] * c);
-        if (v != R(0)) j_add<R>(g, g.J[d] + base + i + g.sy * j + g.sz * k, v);
+        if (v != R(0)) j_add<R, DET>(g, g.J[d] + base + i + g.sy * j + g.sz * k, v);
       }
     }
     if (lane == 0) {
@@ -366,8 +366,8 @@ bool launch_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) 
     // tile kernels, then the particles they listed, one warp each
     launch_tile_kernels<R>(g, a, ORDER, mode, c);
     ScopedPhase ph(c, kPhaseStray);
-    k_deposit_list_warp<R, ORDER><<<c.sm_count * 64, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list,
-                                                                        a.stray_count, a.deactivated);
+    auto klist = g.fix_scale[0] != 0.0 ? k_deposit_list_warp<R, ORDER, 1> : k_deposit_list_warp<R, ORDER, 0>;
+    klist<<<c.sm_count * 64, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count, a.deactivated);
     c.launches += 1;
     return true;
   }

@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <map>
 #include <string>
 #include <utility>
 #include <vector>
@@ -98,11 +99,31 @@ struct Sim : SimBase {
   SortScratch scratch;
   int64_t step_count = 0;
   int64_t step_launches = 0;   // kernels launched by pic_step / pic_sort_now
+  // CUDA graphs (kernel-launch latency dominates once the kernels are fast): every time step
+  // is captured once per "signature" (does it sort; which physical arrays hold what) and replayed as ONE
+  // graph launch afterwards; the signatures of a run repeat with period 2 x sort_interval
+  struct StepGraph {
+    cudaGraphExec_t exec = nullptr;
+    int64_t launches = 0;                    // kernels inside
+    std::vector<Species<R>> after;           // host-side state the step leaves behind (buffer flips, pointer swaps)
+  };
+  std::map<std::vector<uint64_t>, StepGraph> graphs;
+  bool use_graph = true;
+  cudaStream_t cap_stream = nullptr;         // capture only (nothing ever runs on it); replays go to ctx.stream
+  int64_t eager_steps = 0;                   // the first step of a handle runs eagerly (function attributes, first sort)
   unsigned long long* d_deact = nullptr;
   int* d_flags = nullptr;
   double* d_red = nullptr;   // 8 doubles of reduction scratch
+  void drop_graphs() {
+    for (auto& kv : graphs)
+      if (kv.second.exec) cudaGraphExecDestroy(kv.second.exec);
+    graphs.clear();
+    eager_steps = 0;
+  }
   ~Sim() override {
     cudaStreamSynchronize(ctx.stream);
+    drop_graphs();
+    if (cap_stream) cudaStreamDestroy(cap_stream);
     ctx.timer.destroy();
     pool.release();
     cudaGetLastError();
@@ -137,6 +158,7 @@ struct Sim : SimBase {
     sort_interval = o.sort_interval;
     deposit_mode = o.deposit_mode;
     deterministic = o.deterministic != 0;
+    use_graph = o.cuda_graph != 0;
     ctx.stream = (cudaStream_t)o.cuda_stream;
     PIC_CUDA(cudaGetDevice(&ctx.device));
     PIC_CUDA(cudaDeviceGetAttribute(&ctx.sm_count, cudaDevAttrMultiProcessorCount, ctx.device));
@@ -198,6 +220,11 @@ struct Sim : SimBase {
     if (!d_deact || !d_flags || !d_red) return fail(PIC_ERR_OOM, "scratch allocation failed");
     PIC_CUDA(cudaMemsetAsync(d_deact, 0, sizeof(unsigned long long), ctx.stream));
     PIC_CUDA(cudaStreamSynchronize(ctx.stream));
+    if (use_graph && cudaStreamCreateWithFlags(&cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+      cudaGetLastError();
+      cap_stream = nullptr;
+      use_graph = false;
+    }
     return PIC_OK;
   }
 
@@ -264,6 +291,7 @@ struct Sim : SimBase {
     if (n >= ((int64_t)1 << 31)) return fail(PIC_ERR_INVALID_ARG, "more than 2^31-1 particles in one species");
     for (int a = 0; a < 7; ++a)
       if (n > 0 && !arr[a]) return fail(PIC_ERR_INVALID_ARG, "null particle array");
+    drop_graphs();   // the species list and the scratch buffers are part of every captured step
     Species<R> sp;
     sp.q = q;
     sp.m = m;
@@ -411,44 +439,106 @@ struct Sim : SimBase {
     }
   }
 
-  int step(int n) override {
-    if (n < 0) return fail(PIC_ERR_INVALID_ARG, "negative step count");
-    const size_t jbytes = (size_t)g.padded_total() * 3 * sizeof(R);
-    int loB[3], hiB[3], loE[3], hiE[3], lo0[3], hi0[3];
+  struct StepBounds { int loB[3], hiB[3], loE[3], hiE[3], lo0[3], hi0[3]; };
+  StepBounds step_bounds() const {
+    StepBounds b;
     for (int d = 0; d < 3; ++d) {
-      lo0[d] = 0; hi0[d] = g.N[d];
+      b.lo0[d] = 0; b.hi0[d] = g.N[d];
       // Yee: the second B half-step reads E one layer up; CKC also reads one layer to every side, so its
       // E update is widened to [-1, N+2) and its first B half-step to [-2, N+2) (guards are 4 deep)
       const int wide = g.solver == PIC_SOLVER_CKC ? 2 : 1;
-      loB[d] = g.periodic[d] ? -wide : 0;
-      hiB[d] = g.periodic[d] ? g.N[d] + wide : g.N[d];
-      loE[d] = g.periodic[d] ? -(wide - 1) : 0;
-      hiE[d] = hiB[d];
+      b.loB[d] = g.periodic[d] ? -wide : 0;
+      b.hiB[d] = g.periodic[d] ? g.N[d] + wide : g.N[d];
+      b.loE[d] = g.periodic[d] ? -(wide - 1) : 0;
+      b.hiE[d] = b.hiB[d];
     }
+    return b;
+  }
+
+  // one time step: issues every launch on ctx.stream and advances the host-side state
+  void step_body(const StepBounds& b) {
+    const size_t jbytes = (size_t)g.padded_total() * 3 * sizeof(R);
+    if (sort_interval > 0 && step_count % sort_interval == 0) {
+      ScopedPhase ph(ctx, kPhaseSort);
+      do_sort();
+    }
+    {
+      ScopedPhase ph(ctx, kPhaseFields);
+      cudaMemsetAsync(g.J[0], 0, jbytes, ctx.stream);   // the three J arrays are contiguous
+      if (deterministic) cudaMemsetAsync(g.Jfix[0], 0, (size_t)g.padded_total() * 6 * sizeof(long long), ctx.stream);
+    }
+    for (auto& sp : species) particle_step(sp);         // timed per kernel in particles.cu
+    {
+      ScopedPhase ph(ctx, kPhaseFields);
+      if (deterministic && g.fix_scale[0] != 0.0) launch_fix_to_J<R>(g, ctx);   // integer sums -> J
+      launch_fold_J<R>(g, ctx);                    // SumBoundary
+      launch_fill_guards<R>(g, g.J, 3, ctx);       // J images for the widened E update
+      launch_push_B<R>(g, b.loB, b.hiB, ctx);      // widened by one layer on periodic axes, so
+      launch_push_E<R>(g, b.loE, b.hiE, ctx);      // the valid region never reads a stale guard
+      launch_push_B<R>(g, b.lo0, b.hi0, ctx);
+      launch_fill_guards<R>(g, g.F, 6, ctx);       // FillBoundary
+    }
+    step_count++;
+  }
+
+  // what a captured step depends on besides the (fixed) grid: does it sort, and which arrays play which role
+  std::vector<uint64_t> signature() const {
+    std::vector<uint64_t> v;
+    v.push_back(sort_interval > 0 && step_count % sort_interval == 0);
+    for (const auto& sp : species) {
+      v.push_back((uint64_t)sp.cur | ((uint64_t)sp.sorted_once << 1));
+      for (int b = 0; b < 2; ++b) {
+        v.push_back((uint64_t)(uintptr_t)sp.buf[b].x);
+        v.push_back((uint64_t)(uintptr_t)sp.buf[b].y);
+        v.push_back((uint64_t)(uintptr_t)sp.buf[b].z);
+      }
+    }
+    return v;
+  }
+
+  int step(int n) override {
+    if (n < 0) return fail(PIC_ERR_INVALID_ARG, "negative step count");
+    const StepBounds b = step_bounds();
     const int64_t launches0 = ctx.launches;
     for (int s = 0; s < n; ++s) {
-      if (sort_interval > 0 && step_count % sort_interval == 0) {
-        ScopedPhase ph(ctx, kPhaseSort);
-        do_sort();
+      // eager: per-kernel timing is on, graphs are off, or this is the handle's first step
+      if (!use_graph || ctx.timer.on || eager_steps < 1) {
+        step_body(b);
+        eager_steps++;
+        if (ctx.timer.spans.size() > 3000) ctx.timer.fold_completed();   // never waits: pic_step stays asynchronous
+        continue;
       }
-      {
-        ScopedPhase ph(ctx, kPhaseFields);
-        cudaMemsetAsync(g.J[0], 0, jbytes, ctx.stream);   // the three J arrays are contiguous
-        if (deterministic) cudaMemsetAsync(g.Jfix[0], 0, (size_t)g.padded_total() * 6 * sizeof(long long), ctx.stream);
+      const std::vector<uint64_t> sig = signature();
+      auto it = graphs.find(sig);
+      if (it == graphs.end()) {
+        const int64_t l0 = ctx.launches;
+        cudaStream_t user = ctx.stream;
+        if (cudaStreamBeginCapture(cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+          cudaGetLastError();
+          use_graph = false;
+          step_body(b);
+          continue;
+        }
+        ctx.stream = cap_stream;
+        step_body(b);                              // recorded, not run; the host-side state moves on
+        ctx.stream = user;
+        cudaGraph_t gr = nullptr;
+        StepGraph sg;
+        cudaError_t e = cudaStreamEndCapture(cap_stream, &gr);
+        if (e == cudaSuccess) e = cudaGraphInstantiate(&sg.exec, gr, 0);
+        if (gr) cudaGraphDestroy(gr);
+        if (e != cudaSuccess) return cuda_fail(e, "CUDA graph capture of a time step");
+        sg.launches = ctx.launches - l0;
+        ctx.launches = l0;
+        sg.after = species;
+        it = graphs.emplace(sig, std::move(sg)).first;
+      } else {
+        species = it->second.after;
+        step_count++;
       }
-      for (auto& sp : species) particle_step(sp);         // timed per kernel in particles.cu
-      {
-        ScopedPhase ph(ctx, kPhaseFields);
-        if (deterministic && g.fix_scale[0] != 0.0) launch_fix_to_J<R>(g, ctx);   // integer sums -> J
-        launch_fold_J<R>(g, ctx);                    // SumBoundary
-        launch_fill_guards<R>(g, g.J, 3, ctx);       // J images for the widened E update
-        launch_push_B<R>(g, loB, hiB, ctx);          // widened by one layer on periodic axes, so
-        launch_push_E<R>(g, loE, hiE, ctx);          // the valid region never reads a stale guard
-        launch_push_B<R>(g, lo0, hi0, ctx);
-        launch_fill_guards<R>(g, g.F, 6, ctx);       // FillBoundary
-      }
-      step_count++;
-      if (ctx.timer.spans.size() > 3000) ctx.timer.fold_completed();   // never waits: pic_step stays asynchronous
+      cudaError_t e = cudaGraphLaunch(it->second.exec, ctx.stream);
+      if (e != cudaSuccess) return cuda_fail(e, "cudaGraphLaunch");
+      ctx.launches += it->second.launches;
     }
     step_launches += ctx.launches - launches0;
     return check_launch("pic_step launch");
@@ -623,6 +713,7 @@ void pic_default_options(pic_options* o) {
   o->gather_mode = PIC_GATHER_UNIFORM;
   o->solver = PIC_SOLVER_YEE;
   o->deterministic = 0;
+  o->cuda_graph = 1;
   o->cuda_stream = nullptr;
 }
 
@@ -640,7 +731,8 @@ int pic_create(const int32_t n_cells[3], const double dx[3], double dt, int shap
   if (prec != PIC_F64 && prec != PIC_F32) return bad(PIC_ERR_INVALID_ARG, "unknown precision");
   if (o.sort_interval < 0 || o.sort_key_mode < 0 || o.sort_key_mode > 1 || o.deposit_mode < 0 ||
       o.deposit_mode > 5 || o.pusher < 0 || o.pusher > 1 || o.gather_mode < 0 || o.gather_mode > 1 ||
-      o.solver < 0 || o.solver > 1 || o.deterministic < 0 || o.deterministic > 1)
+      o.solver < 0 || o.solver > 1 || o.deterministic < 0 || o.deterministic > 1 ||
+      o.cuda_graph < 0 || o.cuda_graph > 1)
     return bad(PIC_ERR_INVALID_ARG, "bad option value");
   double s2 = 0;
   for (int d = 0; d < 3; ++d) {

@@ -542,7 +542,7 @@ struct CFrag {
   }
 };
 
-template <class R, int ORDER, int NWARP, int MINB>
+template <class R, int ORDER, int NWARP, int MINB, int DET>
 __global__ void __launch_bounds__(NWARP * 32, MINB)
     k_deposit_mma(Grid<R> g, Particles<R> p, R* __restrict__ xn, R* __restrict__ yn, R* __restrict__ zn,
                   const int32_t* __restrict__ tile_start, TileSpec ts, int32_t* __restrict__ stray_list,
@@ -602,9 +602,9 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
           if (cok[b][c]) {
-            if (C.x[b][c] != 0.0) j_add<R>(g, g.J[0] + base + coff[b][c], (R)C.x[b][c]);
-            if (C.y[b][c] != 0.0) j_add<R>(g, g.J[1] + base + coff[b][c], (R)C.y[b][c]);
-            if (C.z[b][c] != 0.0) j_add<R>(g, g.J[2] + base + coff[b][c], (R)C.z[b][c]);
+            if (C.x[b][c] != 0.0) j_add<R, DET>(g, g.J[0] + base + coff[b][c], (R)C.x[b][c]);
+            if (C.y[b][c] != 0.0) j_add<R, DET>(g, g.J[1] + base + coff[b][c], (R)C.y[b][c]);
+            if (C.z[b][c] != 0.0) j_add<R, DET>(g, g.J[2] + base + coff[b][c], (R)C.z[b][c]);
           }
           C.x[b][c] = 0; C.y[b][c] = 0; C.z[b][c] = 0;
         }
@@ -768,13 +768,11 @@ __global__ void __launch_bounds__(NWARP * 32, 1)
   extern __shared__ __align__(16) unsigned char smem_raw[];
   R* box = reinterpret_cast<R*>(smem_raw);   // [6][E (x)][SX: E (z) x E (y), padded]
   R* rec_all = box + 6 * VOL;
-  __shared__ int s_drift[MAXD];
-  __shared__ int s_ndrift;
+  __shared__ int s_drift[NWARP][MAXD];   // per warp, in processing order: nothing here depends on timing
 
   const int tile = blockIdx.x;
   const int s = tile_start[tile], e = tile_start[tile + 1];
   if (s >= e) return;
-  if (threadIdx.x == 0) s_ndrift = 0;
   int tb[3];
   tile_coords(ts, tile, tb);
   const int o0 = tb[0] - PB::HB, o1 = tb[1] - PB::HB, o2 = tb[2] - PB::HB;   // node of local (0,0,0)
@@ -853,20 +851,20 @@ __global__ void __launch_bounds__(NWARP * 32, 1)
   asm volatile("cp.async.wait_all;" ::: "memory");
   __syncthreads();
 
+  int ndrift = 0;   // entries of this warp's list (warp-uniform)
 #pragma unroll 1
   for (int phase = 0; phase < 2; ++phase) {
-    int r_begin = wb, r_end = we, r_step = 32;
+    int r_begin = wb, r_end = we;
     if (phase == 1) {
-      __syncthreads();                                   // every warp's drifted particles are listed
-      r_begin = 32 * warp;
-      r_end = min(s_ndrift, MAXD);
-      r_step = 32 * NWARP;
+      __syncwarp();
+      r_begin = 0;
+      r_end = ndrift;
     }
 #pragma unroll 1
-    for (int rb = r_begin; rb < r_end; rb += r_step) {
+    for (int rb = r_begin; rb < r_end; rb += 32) {
       bool valid = rb + lane < r_end;
       int tp = rb + lane;
-      if (phase == 1) tp = valid ? s_drift[tp] : 0;
+      if (phase == 1) tp = valid ? s_drift[warp][tp] : 0;
       bool elig = false;
       R x1[3] = {0, 0, 0};
       R w = 0;
@@ -876,13 +874,13 @@ __global__ void __launch_bounds__(NWARP * 32, 1)
         prefetch_l2(p.ux + tp + 32); prefetch_l2(p.uy + tp + 32); prefetch_l2(p.uz + tp + 32);
         prefetch_l2(p.w + tp + 32);
       }
+      R x0[3], u[3], wn[3][ORDER + 1], xi0[3], Ef[3], Bf[3];
+      int ln[3];
+      bool drifted = false;
       if (valid) {
-        const R x0[3] = {p.x[tp], p.y[tp], p.z[tp]};
-        R u[3] = {p.ux[tp], p.uy[tp], p.uz[tp]};
+        x0[0] = p.x[tp]; x0[1] = p.y[tp]; x0[2] = p.z[tp];
+        u[0] = p.ux[tp]; u[1] = p.uy[tp]; u[2] = p.uz[tp];
         w = p.w[tp];
-        R wn[3][ORDER + 1], xi0[3];
-        int ln[3];
-        R Ef[3], Bf[3];
         bool inbox = phase == 0;
         {
           R ws[3][ORDER + 1];
@@ -908,19 +906,24 @@ __global__ void __launch_bounds__(NWARP * 32, 1)
             Bf[2] = interp_box<R, ORDER, NS, NS, NN>(box + 5 * VOL, SX * ls[0] + ls[1] + E * l2, ws[0], ws[1], wn[2]);
           }
         }
-        if (!inbox) {
-          // drifted out of the tile's box since the last sort: second pass (gather from global memory with all
-          // lanes busy); in line if the list is full
-          int slot = MAXD;
-          if (phase == 0) slot = atomicAdd(&s_ndrift, 1);
-          if (slot < MAXD) {
-            s_drift[slot] = tp;
+        drifted = !inbox;
+      }
+      // drifted out of the tile's box since the last sort: listed (per warp, in order) for the second pass,
+      // which gathers from global memory with all lanes busy; in line if the list is full
+      if (phase == 0) {
+        const unsigned dm = __ballot_sync(0xffffffffu, drifted);
+        if (dm) {
+          const int slot = ndrift + __popc(dm & ((1u << lane) - 1u));
+          if (drifted && slot < MAXD) {
+            s_drift[warp][slot] = tp;
             valid = false;
-          } else {
-            gather6<R, ORDER, GATHER != 0>(g, x0[0], x0[1], x0[2], Ef, Bf);
           }
+          ndrift = min(MAXD, ndrift + __popc(dm));
         }
-        if (valid) {
+      }
+      if (valid) {
+        if (drifted) gather6<R, ORDER, GATHER != 0>(g, x0[0], x0[1], x0[2], Ef, Bf);
+        {
           push_momentum<R>(PUSHER, p.kq, g.inv_c2, Ef, Bf, u);
           advance<R>(g.dt, g.inv_c2, x0, u, x1);
           p.ux[tp] = u[0]; p.uy[tp] = u[1]; p.uz[tp] = u[2];
@@ -1064,7 +1067,8 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, int mo
   const int n_tiles = a.tiles.nt[0] * a.tiles.nt[1] * a.tiles.nt[2];
   constexpr int kW = kDepTileWarps;
   auto kvec = k_deposit_tile<R, ORDER, kW>;
-  auto kmma = k_deposit_mma<R, ORDER, kDepMmaWarps, kDepMmaCtas>;
+  const bool det = g.fix_scale[0] != 0.0;
+  auto kmma = det ? k_deposit_mma<R, ORDER, kDepMmaWarps, kDepMmaCtas, 1> : k_deposit_mma<R, ORDER, kDepMmaWarps, kDepMmaCtas, 0>;
   constexpr int mw = kDepMmaWarps;
   const size_t push_smem = (size_t)6 * PushBox<ORDER>::VOL * sizeof(R);
   const size_t vec_smem = (size_t)kW * 32 * TWin<ORDER>::REC * sizeof(R);

@@ -539,6 +539,28 @@ def test_deterministic_deposition_is_bit_identical_run_to_run(mode):
     compare_state(o, g, 50 * TOL64)
 
 
+def test_cuda_graph_replay_equals_kernel_by_kernel():
+    """pic_options.cuda_graph: replaying each time step as one captured graph gives the same bits as launching
+    its kernels one by one (deterministic deposition makes the comparison exact), over more than one period
+    of the buffer arrangement (2 x sort_interval steps), with two species and a pic_sort_now in between."""
+    cfg = small("C5", (16, 16, 16), order=3)
+    out = []
+    for graph in (True, False):
+        _, g, _ = make_pair(cfg, fields="random", with_oracle=False, gpu_kwargs=dict(deterministic=True, cuda_graph=graph))
+        g.step(11)
+        g.sort_now()
+        g.step(9)
+        d = g.diagnostics()
+        out.append((g.get_fields(), [g.get_particles(s) for s in range(2)], d["step_launches"], d["steps"]))
+    for grp in range(3):
+        for a, b in zip(out[0][0][grp], out[1][0][grp]):
+            assert np.array_equal(a, b)
+    for s in range(2):
+        for k in ("id", "x", "y", "z", "ux", "uy", "uz", "w"):
+            assert np.array_equal(out[0][1][s][k], out[1][1][s][k]), k
+    assert out[0][2] == out[1][2] and out[0][3] == out[1][3] == 20      # the launch count is the kernels' either way
+
+
 def test_deterministic_deposition_fp32_and_two_species():
     """The same in fp32 (the fixed-point parts are formed from the float contribution in double) with two
     species, whose bounds add up in the fixed-point scale."""
