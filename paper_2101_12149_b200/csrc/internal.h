@@ -108,7 +108,7 @@ constexpr int kPushTileThreads = 256;   // k_push_tile: threads per CTA (one CTA
 constexpr int kDepMmaWarps = 4;         // k_deposit_mma: warps per CTA (one CTA per tile) ...
 constexpr int kDepMmaCtas = 5;          // ... and CTAs per SM the register budget is set for (20 warps per SM)
 constexpr int kFusedWarps = 12;         // k_fused_mma: warps per CTA (one CTA per tile, one per SM: box + 12 record buffers = 216 KB)
-constexpr int kFusedMaxDrift = 1024;    // ... and the drifted particles a CTA lists for its second pass
+constexpr int kFusedMaxDrift = 64;      // ... and the drifted particles each WARP lists for its second pass (12 x 64 x 4 B = 3 KB static)
 constexpr int kDepTileWarps = 8;        // k_deposit_tile: warps per CTA (one CTA per tile, two per SM)
 template <class R>
 struct ParticleStep {

@@ -272,6 +272,157 @@ __device__ __forceinline__ void axis_window(R xi0, R xi1, int& cell, R* S0, R* D
   axis_window_from<R, ORDER, NW, BL>(l0, w0, xi0, xi1, cell, S0, DS, fits);
 }
 
+// The y and z windows are tied to the old cell and hold exactly the moves that stay in it. A particle that
+// crosses ONE cell face along the axis has a new support that sticks out of the window by one node, below
+// (ext = 1, window slot -1) or above (ext = 2, slot NW), where its old weight is zero and its new one is
+// `dext`; the NW window slots are filled as always (DS = new - old, the new weights shifted by one slot).
+// Esirkepov's J is a sum over nodes that is linear in the pair (S0, DS) of every single node, so the window
+// part goes through the tile kernels' contractions unchanged and the one extra node is added separately
+// (extra_node_deposit below). ext = 0: fits; ext = 3: further out (per-particle pass).
+template <class R, int ORDER, int NW, int BL>
+__device__ __forceinline__ void axis_window_ext(R xi0, R xi1, int& cell, R* S0, R* DS, int& ext, R& dext) {
+  R w0[ORDER + 1], w1[ORDER + 1];
+  const int l0 = shape<R, ORDER>(xi0, w0);
+  const int l1 = shape<R, ORDER>(xi1, w1);
+  const int c = ORDER == 2 ? (int)floor(xi0) : (ORDER == 1 ? l0 : l0 + 1);
+  cell = c;
+  const int so0 = l0 - (c - BL);   // static for orders 1 and 3
+  const int sl1 = l1 - (c - BL);
+  if constexpr (ORDER != 2 && NW == ORDER + 1) {
+    // tight window: it is the old support itself; the new one starts at slot -1, 0 or +1
+    const int sh = l1 - l0;
+#pragma unroll
+    for (int i = 0; i < NW; ++i) {
+      const R up = i >= 1 ? w1[i >= 1 ? i - 1 : 0] : R(0);          // sh = +1
+      const R dn = i + 1 < NW ? w1[i + 1 < NW ? i + 1 : 0] : R(0);  // sh = -1
+      const R b = sh == 0 ? w1[i] : (sh > 0 ? up : dn);
+      S0[i] = w0[i];
+      DS[i] = sub_rn(b, w0[i]);
+    }
+    ext = sh == 0 ? 0 : (sh == -1 ? 1 : (sh == 1 ? 2 : 3));
+    dext = sh < 0 ? w1[0] : w1[ORDER];
+    return;
+  }
+#pragma unroll
+  for (int i = 0; i < NW; ++i) {
+    R a = 0, b = 0;
+#pragma unroll
+    for (int k = 0; k <= ORDER; ++k) {
+      a = (i == so0 + k) ? w0[k] : a;
+      b = (i == sl1 + k) ? w1[k] : b;
+    }
+    S0[i] = a;
+    DS[i] = sub_rn(b, a);
+  }
+  const bool oldfits = (so0 >= 0) & (so0 + ORDER < NW);
+  const bool fits = (sl1 >= 0) & (sl1 + ORDER < NW);
+  ext = !oldfits ? 3 : (fits ? 0 : (sl1 == -1 ? 1 : (sl1 + ORDER == NW ? 2 : 3)));
+  dext = sl1 < 0 ? w1[0] : w1[ORDER];
+}
+
+// The extra node of the particles of a round that crossed a face in y or in z (axis_window_ext): for each
+// of them the warp adds the contributions of that one node, lane = (i, m) with i the NX window nodes along x
+// (fastest: contiguous reductions) and m the window slots of the other transverse axis. At the extra node
+// the old weight is 0 and the new one d, hence with (S0, DS) = (0, d) along the crossing axis e, o the other
+// transverse axis and A = S0x + DSx/2, B = S0x/2 + DSx/3 (all in the particle's record):
+//   Jx = PX[i] d (S0o[m]/2 + DSo[m]/3),   Jo = Po[m] d B[i],   Je = f_e (running sum of DS_e) (A[i] S0o[m] + B[i] DSo[m]),
+// the running sum through the extra node being d below the window and the total, 0, above it.
+// extc: 0 none, 1/2 y below/above, 5/6 z below/above; fext = f_e d for a node below, else 0. Warp-uniform.
+// Nothing but extc is kept across the contraction: the owning lane recomputes d (same expression, same bits)
+// from the new position it still holds for the store.
+template <class R, int ORDER, int DET, class W>
+__device__ __forceinline__ void extra_node_deposit_warp(const Grid<R>& g, const R* __restrict__ rec, unsigned em, int extc,
+                                                     R x1y, R x1z, R w, const R* jf, int wx0, int wy0, int wz0) {
+  constexpr int NX = W::NX, NYZ = W::NYZ;
+  const int lane = threadIdx.x & 31;
+  const R half = R(0.5), third = R(1) / R(3);
+  R dext = 0, fext = 0;
+  if (extc != 0) {
+    const int e = extc < 4 ? 1 : 2;
+    R w1[ORDER + 1];
+    shape<R, ORDER>(mul_rn(e == 1 ? x1y : x1z, g.inv_dx[e]), w1);
+    const bool below = (extc & 3) == 1;
+    dext = below ? w1[0] : w1[ORDER];
+    fext = below ? -(w * jf[e]) * dext : R(0);
+  }
+  while (em) {
+    const int src = __ffs(em) - 1;
+    em &= em - 1;
+    const int ec = __shfl_sync(0xffffffffu, extc, src);
+    const R d = __shfl_sync(0xffffffffu, dext, src);
+    const R fe = __shfl_sync(0xffffffffu, fext, src);
+    const int X0 = __shfl_sync(0xffffffffu, wx0, src), Y0 = __shfl_sync(0xffffffffu, wy0, src),
+              Z0 = __shfl_sync(0xffffffffu, wz0, src);
+    if (lane < NX * NYZ) {
+      const R* rr = rec + src * W::REC;
+      const int i = lane % NX, m = lane / NX;
+      const bool isy = ec < 4;
+      const int eo = (ec & 3) == 1 ? -1 : NYZ;
+      const Pair2<R> ab = *reinterpret_cast<const Pair2<R>*>(rr + W::oAB + 2 * i);
+      const R px = rr[W::oPX + i];
+      const Pair2<R> ov = *reinterpret_cast<const Pair2<R>*>(rr + (isy ? W::oZ : W::oY) + 2 * m);
+      const R po = rr[(isy ? W::oPZ : W::oPY) + m];
+      const R vx = px * (d * (half * ov.a + third * ov.b));
+      const R vo = po * (d * ab.b);
+      const R ve = fe * (ab.a * ov.a + ab.b * ov.b);
+      const int base = g.idx(X0 + i, isy ? Y0 + eo : Y0 + m, isy ? Z0 + m : Z0 + eo);
+      if (vx != R(0)) j_add<R, DET>(g, g.J[0] + base, vx);
+      if (vo != R(0)) j_add<R, DET>(g, g.J[isy ? 2 : 1] + base, vo);
+      if (ve != R(0)) j_add<R, DET>(g, g.J[isy ? 1 : 2] + base, ve);
+    }
+  }
+}
+
+template <class R, int ORDER, int DET, class W>
+__device__ __forceinline__ void extra_node_deposit(const Grid<R>& g, const R* __restrict__ rec, int extc, R x1y, R x1z,
+                                                   R w, const R* jf, int wx0, int wy0, int wz0) {
+  const unsigned em = __ballot_sync(0xffffffffu, extc != 0);
+  if (em != 0) extra_node_deposit_warp<R, ORDER, DET, W>(g, rec, em, extc, x1y, x1z, w, jf, wx0, wy0, wz0);
+}
+
+
+// One particle's record (layout W: {A_x,B_x}[NX] | PX[NX] | {S0_y,DS_y}[NYZ] | PY[NYZ] | {S0_z,DS_z}[NYZ] | PZ[NYZ]),
+// written axis by axis as soon as the axis is known, so that only one axis' weights are live at a time
+// (a record whose particle turns out not to fit is simply never read). Returns the cell of the old
+// position in c[], whether the move fits the windows (x: +-1 cell; y, z: same cell, or ONE face of ONE
+// of the two crossed) and in `extc` the extra node of such a crossing (extra_node_deposit).
+template <class R, int ORDER, class W>
+__device__ __forceinline__ bool build_record(const Grid<R>& g, const R* jf, R* __restrict__ rr, const R* x0,
+                                             const R* x1, R w, int* c, int& extc) {
+  constexpr int NX = W::NX, NYZ = W::NYZ;
+  const R half = R(0.5), third = R(1) / R(3);
+  bool fitx;
+  {
+    R S0[NX], DS[NX];
+    axis_window<R, ORDER, NX, W::BLX>(mul_rn(x0[0], g.inv_dx[0]), mul_rn(x1[0], g.inv_dx[0]), c[0], S0, DS, fitx);
+    const R fx = -(w * jf[0]);
+    R px = 0;
+#pragma unroll
+    for (int i = 0; i < NX; ++i) {
+      *reinterpret_cast<Pair2<R>*>(rr + W::oAB + 2 * i) = Pair2<R>{S0[i] + half * DS[i], half * S0[i] + third * DS[i]};
+      px += DS[i];
+      rr[W::oPX + i] = fx * px;
+    }
+  }
+  int e[2];
+#pragma unroll
+  for (int a = 0; a < 2; ++a) {   // y, z
+    R S0[NYZ], DS[NYZ], d;
+    axis_window_ext<R, ORDER, NYZ, W::BLYZ>(mul_rn(x0[1 + a], g.inv_dx[1 + a]), mul_rn(x1[1 + a], g.inv_dx[1 + a]),
+                                            c[1 + a], S0, DS, e[a], d);
+    const R f = -(w * jf[1 + a]);
+    R pr = e[a] == 1 ? d : R(0);   // running sum of DS: a node below the window comes first
+    const int oS = a == 0 ? W::oY : W::oZ, oP = a == 0 ? W::oPY : W::oPZ;
+#pragma unroll
+    for (int i = 0; i < NYZ; ++i) {
+      *reinterpret_cast<Pair2<R>*>(rr + oS + 2 * i) = Pair2<R>{S0[i], DS[i]};
+      pr += DS[i];
+      rr[oP + i] = f * pr;
+    }
+  }
+  extc = e[0] ? e[0] : (e[1] ? 4 + e[1] : 0);
+  return fitx & (e[0] < 3) & (e[1] < 3) & ((e[0] == 0) | (e[1] == 0));
+}
 
 // Register accumulators of one lane: the (j,k) column of a window of NX nodes along x, three
 // components. The slot of box node X is X mod NX, so when the window advances by one cell nothing
@@ -321,20 +472,20 @@ __device__ __forceinline__ R group_sum(R v) {
 
 // one physical slot (static P), summed over the groups -> the J element jx points at, then cleared.
 // Warp-uniform.
-template <class R, int ORDER, int P>
+template <class R, int ORDER, int P, int DET>
 __device__ __forceinline__ void flush_slot(const Grid<R>& g, Acc<R, TWin<ORDER>::NX>& a, const JPtr<R>& jx, bool writer) {
   using W = TWin<ORDER>;
   const R vx = group_sum<R, W::LG>(a.x[P]), vy = group_sum<R, W::LG>(a.y[P]), vz = group_sum<R, W::LG>(a.z[P]);
   if (writer) {
-    if (vx != R(0)) j_add<R>(g, jx.p[0], vx);
-    if (vy != R(0)) j_add<R>(g, jx.p[1], vy);
-    if (vz != R(0)) j_add<R>(g, jx.p[2], vz);
+    if (vx != R(0)) j_add<R, DET>(g, jx.p[0], vx);
+    if (vy != R(0)) j_add<R, DET>(g, jx.p[1], vy);
+    if (vz != R(0)) j_add<R, DET>(g, jx.p[2], vz);
   }
   a.x[P] = 0; a.y[P] = 0; a.z[P] = 0;
 }
 
 // all slots: physical slot p holds logical slot (p - ph) mod NX of the window at jx. Warp-uniform.
-template <class R, int ORDER>
+template <class R, int ORDER, int DET>
 __device__ __forceinline__ void flush_window(const Grid<R>& g, Acc<R, TWin<ORDER>::NX>& a, const JPtr<R>& jx, int ph, bool writer) {
   using W = TWin<ORDER>;
   constexpr int NX = W::NX;
@@ -344,9 +495,9 @@ __device__ __forceinline__ void flush_window(const Grid<R>& g, Acc<R, TWin<ORDER
     i += i < 0 ? NX : 0;
     const R vx = group_sum<R, W::LG>(a.x[p]), vy = group_sum<R, W::LG>(a.y[p]), vz = group_sum<R, W::LG>(a.z[p]);
     if (writer) {
-      if (vx != R(0)) j_add<R>(g, jx.p[0] + i, vx);
-      if (vy != R(0)) j_add<R>(g, jx.p[1] + i, vy);
-      if (vz != R(0)) j_add<R>(g, jx.p[2] + i, vz);
+      if (vx != R(0)) j_add<R, DET>(g, jx.p[0] + i, vx);
+      if (vy != R(0)) j_add<R, DET>(g, jx.p[1] + i, vy);
+      if (vz != R(0)) j_add<R, DET>(g, jx.p[2] + i, vz);
     }
   }
   a.zero();
@@ -354,26 +505,27 @@ __device__ __forceinline__ void flush_window(const Grid<R>& g, Acc<R, TWin<ORDER
 
 // the particles of one cell (cnt of them, record slots listed in order[]): NG at a time, one per
 // group. PH = (first box node of the cell's window) mod NX; adv = the window moved up one cell.
-template <class R, int ORDER, int PH>
+template <class R, int ORDER, int PH, int DET>
 __device__ __forceinline__ void cell_batch(const Grid<R>& g, Acc<R, TWin<ORDER>::NX>& a, bool adv, const JPtr<R>& jx_old, bool writer,
                                            const R* __restrict__ rec, const int* __restrict__ order, int cnt, int grp,
                                            int j, int k) {
   using W = TWin<ORDER>;
   constexpr int NX = W::NX, NG = 32 / W::LG;
-  if (adv) flush_slot<R, ORDER, (PH + NX - 1) % NX>(g, a, jx_old, writer);
+  if (adv) flush_slot<R, ORDER, (PH + NX - 1) % NX, DET>(g, a, jx_old, writer);
 #pragma unroll 1
   for (int it = grp; it < cnt; it += NG) accumulate<R, ORDER, PH>(a, rec + order[it] * W::REC, j, k);
 }
 
 // Every finished window node is one reduction at L2 (RED.ADD.F64 / .F32): no J box in shared memory,
 // no prologue / epilogue, no block barrier, so two 8-warp CTAs per SM overlap freely.
-template <class R, int ORDER, int NWARP>
+template <class R, int ORDER, int NWARP, int DET>
 __global__ void __launch_bounds__(NWARP * 32, 2)
     k_deposit_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn, R* __restrict__ yn, R* __restrict__ zn,
                    const int32_t* __restrict__ tile_start, TileSpec ts, int32_t* __restrict__ stray_list,
                    unsigned int* __restrict__ stray_count, unsigned long long* deactivated) {
   using W = TWin<ORDER>;
   constexpr int NX = W::NX, NYZ = W::NYZ, LG = W::LG, REC = W::REC;
+  constexpr bool kExt = ORDER != 1;   // extra node of a face crossing in y or z taken here (see below)
   extern __shared__ __align__(16) unsigned char smem_raw[];
   R* rec_all = reinterpret_cast<R*>(smem_raw);
   __shared__ int s_order[NWARP][32];
@@ -416,24 +568,39 @@ __global__ void __launch_bounds__(NWARP * 32, 2)
     R x1[3] = {0, 0, 0};
     R w = 0;
     int code = -1;
+    int extc = 0;           // extra node of a particle that crossed a face in y or z (extra_node_deposit)
     if (valid) {
       R x0[3] = {p.x[t], p.y[t], p.z[t]};
       x1[0] = xn[t]; x1[1] = yn[t]; x1[2] = zn[t];
       w = p.w[t];
+      // all three axes first, the record only if the move fits (this kernel has the registers for it; at
+      // order 1 in fp32 that order of things is 20 % faster than build_record's axis-by-axis stores, and the
+      // extra node is left out there: measured on C3, taking it in line costs 0.16 ms and saves 0.05 ms of the
+      // per-particle pass)
       R S0x[NX], DSx[NX], S0y[NYZ], DSy[NYZ], S0z[NYZ], DSz[NYZ];
       int c[3];
-      bool fit[3];
-      axis_window<R, ORDER, NX, W::BLX>(mul_rn(x0[0], g.inv_dx[0]), mul_rn(x1[0], g.inv_dx[0]), c[0], S0x, DSx, fit[0]);
-      axis_window<R, ORDER, NYZ, W::BLYZ>(mul_rn(x0[1], g.inv_dx[1]), mul_rn(x1[1], g.inv_dx[1]), c[1], S0y, DSy, fit[1]);
-      axis_window<R, ORDER, NYZ, W::BLYZ>(mul_rn(x0[2], g.inv_dx[2]), mul_rn(x1[2], g.inv_dx[2]), c[2], S0z, DSz, fit[2]);
+      bool fitx, fityz;
+      int ey = 0, ez = 0;
+      R dy = 0, dz = 0;
+      axis_window<R, ORDER, NX, W::BLX>(mul_rn(x0[0], g.inv_dx[0]), mul_rn(x1[0], g.inv_dx[0]), c[0], S0x, DSx, fitx);
+      if constexpr (kExt) {
+        axis_window_ext<R, ORDER, NYZ, W::BLYZ>(mul_rn(x0[1], g.inv_dx[1]), mul_rn(x1[1], g.inv_dx[1]), c[1], S0y, DSy, ey, dy);
+        axis_window_ext<R, ORDER, NYZ, W::BLYZ>(mul_rn(x0[2], g.inv_dx[2]), mul_rn(x1[2], g.inv_dx[2]), c[2], S0z, DSz, ez, dz);
+        fityz = (ey < 3) & (ez < 3) & ((ey == 0) | (ez == 0));
+      } else {
+        bool fy_, fz_;
+        axis_window<R, ORDER, NYZ, W::BLYZ>(mul_rn(x0[1], g.inv_dx[1]), mul_rn(x1[1], g.inv_dx[1]), c[1], S0y, DSy, fy_);
+        axis_window<R, ORDER, NYZ, W::BLYZ>(mul_rn(x0[2], g.inv_dx[2]), mul_rn(x1[2], g.inv_dx[2]), c[2], S0z, DSz, fz_);
+        fityz = fy_ & fz_;
+      }
       const int rc0 = c[0] - tb[0], rc1 = c[1] - tb[1], rc2 = c[2] - tb[2];
-      elig = fit[0] & fit[1] & fit[2] & (rc0 >= 0) & (rc0 < ts.T[0]) & (rc1 >= 0) & (rc1 < ts.T[1]) & (rc2 >= 0) &
-             (rc2 < ts.T[2]);
+      elig = fitx & fityz & (rc0 >= 0) & (rc0 < ts.T[0]) & (rc1 >= 0) & (rc1 < ts.T[1]) & (rc2 >= 0) & (rc2 < ts.T[2]);
       if (elig) {
         code = ((rc0 | (rc1 << 4) | (rc2 << 8)) << 3) | (rc0 % NX);
+        extc = ey ? ey : (ez ? 4 + ez : 0);
         R* rr = rec + lane * REC;
         const R fx = -(w * p.jf[0]), fy = -(w * p.jf[1]), fz = -(w * p.jf[2]);
-        R px = 0, py = 0, pz = 0;
+        R px = 0, py = ey == 1 ? dy : R(0), pz = ez == 1 ? dz : R(0);
 #pragma unroll
         for (int i = 0; i < NX; ++i) {
           *reinterpret_cast<Pair2<R>*>(rr + W::oAB + 2 * i) =
@@ -465,18 +632,23 @@ __global__ void __launch_bounds__(NWARP * 32, 2)
       const bool adv = ib == cur + 1;
       JPtr<R> jx_old{};
       if (cur != INT_MIN) jx_old = column(cur);
-      if (ib != cur && !adv && cur != INT_MIN) flush_window<R, ORDER>(g, acc, jx_old, curph, grp == 0);
+      if (ib != cur && !adv && cur != INT_MIN) flush_window<R, ORDER, DET>(g, acc, jx_old, curph, grp == 0);
       const int* ord = s_order[warp];
       switch (ph) {
-        case 0: cell_batch<R, ORDER, 0>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 1: cell_batch<R, ORDER, 1>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 2: cell_batch<R, ORDER, 2>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 3: cell_batch<R, ORDER, 3 % NX>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        case 4: cell_batch<R, ORDER, 4 % NX>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
-        default: cell_batch<R, ORDER, 5 % NX>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 0: cell_batch<R, ORDER, 0, DET>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 1: cell_batch<R, ORDER, 1, DET>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 2: cell_batch<R, ORDER, 2, DET>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 3: cell_batch<R, ORDER, 3 % NX, DET>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        case 4: cell_batch<R, ORDER, 4 % NX, DET>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
+        default: cell_batch<R, ORDER, 5 % NX, DET>(g, acc, adv, jx_old, grp == 0, rec, ord, cnt, grp, j, k); break;
       }
       cur = ib;
       curph = ph;
+      __syncwarp();
+    }
+    if constexpr (kExt) {
+      extra_node_deposit<R, ORDER, DET, W>(g, rec, extc, x1[1], x1[2], w, p.jf, b0 + ((code >> 3) & 15),
+                                          b1 + ((code >> 7) & 15), b2 + (code >> 11));
       __syncwarp();
     }
     // particles deposited here are finished: wrap and store; the others go to the list untouched
@@ -499,7 +671,7 @@ __global__ void __launch_bounds__(NWARP * 32, 2)
       xn[t] = x1[0]; yn[t] = x1[1]; zn[t] = x1[2];
     }
   }
-  if (cur != INT_MIN) flush_window<R, ORDER>(g, acc, column(cur), curph, grp == 0);
+  if (cur != INT_MIN) flush_window<R, ORDER, DET>(g, acc, column(cur), curph, grp == 0);
 }
 
 // =================================================================== Esirkepov on the fp64 tensor pipe
@@ -624,6 +796,7 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
     R x1[3] = {0, 0, 0};
     R w = 0;
     int code = -1;
+    int extc = 0;           // extra node of a particle that crossed a face in y or z (extra_node_deposit)
     if (tp + 32 < we) {   // the next round's particle data on its way to L2 while this round computes
       prefetch_l2(p.x + tp + 32); prefetch_l2(p.y + tp + 32); prefetch_l2(p.z + tp + 32);
       prefetch_l2(xn + tp + 32); prefetch_l2(yn + tp + 32); prefetch_l2(zn + tp + 32);
@@ -633,36 +806,16 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
       R x0[3] = {p.x[tp], p.y[tp], p.z[tp]};
       x1[0] = xn[tp]; x1[1] = yn[tp]; x1[2] = zn[tp];
       w = p.w[tp];
-      R S0x[NX], DSx[NX], S0y[NYZ], DSy[NYZ], S0z[NYZ], DSz[NYZ];
       int c[3];
-      bool fit[3];
-      axis_window<R, ORDER, NX, BLX>(mul_rn(x0[0], g.inv_dx[0]), mul_rn(x1[0], g.inv_dx[0]), c[0], S0x, DSx, fit[0]);
-      axis_window<R, ORDER, NYZ, BLYZ>(mul_rn(x0[1], g.inv_dx[1]), mul_rn(x1[1], g.inv_dx[1]), c[1], S0y, DSy, fit[1]);
-      axis_window<R, ORDER, NYZ, BLYZ>(mul_rn(x0[2], g.inv_dx[2]), mul_rn(x1[2], g.inv_dx[2]), c[2], S0z, DSz, fit[2]);
+      int ec;
+      const bool fits = build_record<R, ORDER, W>(g, p.jf, rec + lane * REC, x0, x1, w, c, ec);
       // the cell must be inside the grid and within 4 cells of the tile (4-bit biased offsets)
       const int rc0 = c[0] - tb[0] + 4, rc1 = c[1] - tb[1] + 4, rc2 = c[2] - tb[2] + 4;
-      elig = fit[0] & fit[1] & fit[2] & (((rc0 | rc1 | rc2) & ~15) == 0) & (c[0] >= 0) & (c[0] < g.N[0]) &
-             (c[1] >= 0) & (c[1] < g.N[1]) & (c[2] >= 0) & (c[2] < g.N[2]);
+      elig = fits & (((rc0 | rc1 | rc2) & ~15) == 0) & (c[0] >= 0) & (c[0] < g.N[0]) & (c[1] >= 0) & (c[1] < g.N[1]) &
+             (c[2] >= 0) & (c[2] < g.N[2]);
       if (elig) {
         code = rc0 | (rc1 << 4) | (rc2 << 8);
-        R* rr = rec + lane * REC;
-        const R fx = -(w * p.jf[0]), fy = -(w * p.jf[1]), fz = -(w * p.jf[2]);
-        R px = 0, py = 0, pz = 0;
-#pragma unroll
-        for (int i = 0; i < NX; ++i) {
-          *reinterpret_cast<Pair2<R>*>(rr + W::oAB + 2 * i) =
-              Pair2<R>{S0x[i] + half * DSx[i], half * S0x[i] + third * DSx[i]};
-          px += DSx[i];
-          rr[W::oPX + i] = fx * px;
-        }
-#pragma unroll
-        for (int i = 0; i < NYZ; ++i) {
-          *reinterpret_cast<Pair2<R>*>(rr + W::oY + 2 * i) = Pair2<R>{S0y[i], DSy[i]};
-          *reinterpret_cast<Pair2<R>*>(rr + W::oZ + 2 * i) = Pair2<R>{S0z[i], DSz[i]};
-          py += DSy[i]; pz += DSz[i];
-          rr[W::oPY + i] = fy * py;
-          rr[W::oPZ + i] = fz * pz;
-        }
+        extc = ec;
       }
     }
     __syncwarp();
@@ -715,6 +868,8 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
         }
       }
     }
+    extra_node_deposit<R, ORDER, DET, W>(g, rec, extc, x1[1], x1[2], w, p.jf, tb[0] + (code & 15) - 4 - BLX,
+                                         tb[1] + ((code >> 4) & 15) - 4 - BLYZ, tb[2] + (code >> 8) - 4 - BLYZ);
     __syncwarp();
     // particles deposited here are finished: wrap and store; the others go to the list untouched
     const bool stray = valid && !elig;
@@ -1066,8 +1221,8 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, int mo
   R *xn = a.alt.x, *yn = a.alt.y, *zn = a.alt.z;
   const int n_tiles = a.tiles.nt[0] * a.tiles.nt[1] * a.tiles.nt[2];
   constexpr int kW = kDepTileWarps;
-  auto kvec = k_deposit_tile<R, ORDER, kW>;
   const bool det = g.fix_scale[0] != 0.0;
+  auto kvec = det ? k_deposit_tile<R, ORDER, kW, 1> : k_deposit_tile<R, ORDER, kW, 0>;
   auto kmma = det ? k_deposit_mma<R, ORDER, kDepMmaWarps, kDepMmaCtas, 1> : k_deposit_mma<R, ORDER, kDepMmaWarps, kDepMmaCtas, 0>;
   constexpr int mw = kDepMmaWarps;
   const size_t push_smem = (size_t)6 * PushBox<ORDER>::VOL * sizeof(R);
