@@ -274,7 +274,8 @@ def config_dict(cfg, world, args):
             cfg.n_particles * (7 * (8 if cfg.dtype == "f64" else 4) + 8) / 1e9),
         "deposit_mode": args.deposit_mode,
         "variant": {"pusher": args.pusher, "gather_mode": args.gather_mode, "solver": args.solver,
-                    "deterministic": bool(args.deterministic), "cuda_graph": not args.no_graph},
+                    "deterministic": bool(args.deterministic), "cuda_graph": not args.no_graph,
+                    "box_staging": args.box_staging},
     }
 
 
@@ -318,7 +319,8 @@ def run_ours(args):
     stream = torch.cuda.current_stream()
     kw = dict(dtype=np_dt, periodic=cfg.periodic, tile=cfg.tile, sort_interval=cfg.sort_interval,
               deposit_mode=args.deposit_mode, sort_key_mode=args.sort_key_mode, stream=stream.cuda_stream,
-              pusher=args.pusher, gather_mode=args.gather_mode, solver=args.solver, deterministic=args.deterministic, cuda_graph=not args.no_graph)
+              pusher=args.pusher, gather_mode=args.gather_mode, solver=args.solver, deterministic=args.deterministic, cuda_graph=not args.no_graph,
+              box_staging=args.box_staging)
 
     # ---------------- leg 1: state resident in HBM
     sim = pic.Sim(cfg.n_cells, cfg.dx, cfg.dt, cfg.order, **kw)
@@ -534,6 +536,7 @@ def main(argv=None):
     ap.add_argument("--solver", type=int, default=0, help="variants: PIC_SOLVER_* (0 Yee, 1 CKC)")
     ap.add_argument("--deterministic", action="store_true", help="variants: pic_options.deterministic (integer reductions into J)")
     ap.add_argument("--no-graph", action="store_true", help="variants: launch every kernel of a step separately (pic_options.cuda_graph = 0)")
+    ap.add_argument("--box-staging", type=int, default=0, help="variants: PIC_STAGE_* (0 auto = TMA in fp64, 1 element-wise cp.async, 2 TMA)")
     ap.add_argument("--skip-e2e", action="store_true", help="profiling runs: device-resident leg only")
     ap.add_argument("--skip-cpu", action="store_true", help="profiling runs: do not time the oracle")
     ap.add_argument("--skip-probe", action="store_true", help="profiling runs: one launch per on-chip probe instead of 0.2 s")

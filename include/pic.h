@@ -104,6 +104,13 @@ enum { PIC_GATHER_UNIFORM = 0, PIC_GATHER_GALERKIN = 1 };
  * axes at c*dt = min(dx), which is also its time step limit (PIC_ERR_CFL beyond it). */
 enum { PIC_SOLVER_YEE = 0, PIC_SOLVER_CKC = 1 };
 
+/* How k_push_tile brings a tile's E/B stencil box into shared memory (north_star: "TMA where the box is
+ * regular"; PAPER.md:209-211 contrasts the paper's cached global reads with explicit shared-memory staging).
+ * AUTO: one bulk tensor copy per CTA (cp.async.bulk.tensor, TMA) in fp64 whenever the padded field arrays
+ * meet TMA's 16-byte stride rule (even padded extents), else element-wise cp.async. CP_ASYNC / TMA force one
+ * (TMA silently falls back where the rule is not met). Results are bit-identical either way. */
+enum { PIC_STAGE_AUTO = 0, PIC_STAGE_CP_ASYNC = 1, PIC_STAGE_TMA = 2 };
+
 /* Options; pass NULL to pic_create for the defaults given here. */
 typedef struct {
   int32_t periodic[3];   /* default {1,1,1}; 0 = truncation with zeroed guard cells on that axis:
@@ -131,6 +138,7 @@ typedef struct {
                             (launch latency dominates once the kernels are fast). The first
                             step of a handle, and every step while phase timing is on, is launched kernel
                             by kernel. 0: always kernel by kernel. Results are identical either way. */
+  int32_t box_staging;   /* PIC_STAGE_*; default PIC_STAGE_AUTO */
   void*   cuda_stream;   /* cudaStream_t all work is issued on (e.g. torch's current stream);
                             NULL = the legacy default stream */
 } pic_options;

@@ -17,6 +17,7 @@ PIC_HOST, PIC_DEVICE = 0, 1
 PIC_DEPOSIT_AUTO, PIC_DEPOSIT_GLOBAL, PIC_DEPOSIT_COOP, PIC_DEPOSIT_TILE, PIC_DEPOSIT_TILE_MMA = 0, 1, 2, 3, 4
 PIC_DEPOSIT_FUSED = 5
 PIC_PUSHER_BORIS, PIC_PUSHER_VAY = 0, 1
+PIC_STAGE_AUTO, PIC_STAGE_CP_ASYNC, PIC_STAGE_TMA = 0, 1, 2
 PIC_GATHER_UNIFORM, PIC_GATHER_GALERKIN = 0, 1
 PIC_SOLVER_YEE, PIC_SOLVER_CKC = 0, 1
 PIC_NDIAG = 12
@@ -46,7 +47,8 @@ class pic_options(C.Structure):
     _fields_ = [("periodic", C.c_int32 * 3), ("tile", C.c_int32 * 3), ("sort_interval", C.c_int32),
                 ("sort_key_mode", C.c_int32), ("deposit_mode", C.c_int32), ("pusher", C.c_int32),
                 ("gather_mode", C.c_int32), ("solver", C.c_int32),
-                ("deterministic", C.c_int32), ("cuda_graph", C.c_int32), ("cuda_stream", C.c_void_p)]
+                ("deterministic", C.c_int32), ("cuda_graph", C.c_int32), ("box_staging", C.c_int32),
+                ("cuda_stream", C.c_void_p)]
 
 
 _lib = None
@@ -254,7 +256,7 @@ class Sim:
 
     def __init__(self, n_cells, dx, dt, order, dtype=np.float64, periodic=(1, 1, 1), tile=(8, 8, 8),
                  sort_interval=4, sort_key_mode=0, deposit_mode=PIC_DEPOSIT_AUTO, stream=None,
-                 pusher=PIC_PUSHER_BORIS, gather_mode=PIC_GATHER_UNIFORM, solver=PIC_SOLVER_YEE, deterministic=False, cuda_graph=True):
+                 pusher=PIC_PUSHER_BORIS, gather_mode=PIC_GATHER_UNIFORM, solver=PIC_SOLVER_YEE, deterministic=False, cuda_graph=True, box_staging=0):
         self.dtype = np.dtype(dtype)
         self.n_cells = tuple(int(v) for v in n_cells)
         self.n_valid = self.n_cells[0] * self.n_cells[1] * self.n_cells[2]
@@ -271,6 +273,7 @@ class Sim:
         o.solver = int(solver)
         o.deterministic = 1 if deterministic else 0
         o.cuda_graph = 1 if cuda_graph else 0
+        o.box_staging = int(box_staging)
         o.cuda_stream = stream
         self._h = pic_create(self.n_cells, dx, dt, order, PIC_F64 if self.dtype == np.float64 else PIC_F32, o)
 

@@ -1,5 +1,7 @@
 // Host-side declarations shared by the translation units of libpic.so (CUDA path only).
 #pragma once
+#include <cuda.h>   // CUtensorMap (types only: the encoder is fetched with cudaGetDriverEntryPoint, nothing links libcuda)
+
 #include <set>
 #include <vector>
 
@@ -80,6 +82,10 @@ struct Ctx {
   int device = 0;         // the device the handle was created on
   int sm_count = 148;     // its multiProcessorCount (grid sizing of the grid-stride kernels)
   std::set<const void*> smem_opted;   // kernels whose >48 KB dynamic shared memory opt-in is done for this handle
+  // TMA staging of k_push_tile's E/B box (tile_kernels.cu make_push_tensor_map): one 4-D tensor map over the
+  // six padded field arrays (x, y, z, component); off when the arrays do not meet TMA's 16-byte stride rule
+  bool tma_push = false;
+  alignas(64) CUtensorMap tmap_push;
   int64_t launches = 0;   // kernels launched through this handle
   Timer timer;
 };
@@ -125,6 +131,12 @@ struct ParticleStep {
 // (the caller swaps the position pointers of the two buffer sets), false if updated in place.
 template <class R>
 bool launch_particles(const Grid<R>& g, const ParticleStep<R>& a, int order, int mode, Ctx& c);
+
+// ---- tile_kernels.cu: the tensor map k_push_tile stages its box through (c.tma_push, c.tmap_push); false if
+// TMA cannot describe these arrays (then the kernel copies element by element with cp.async). `stage_mode`:
+// PIC_STAGE_* of pic_options (AUTO = TMA where it applies); tile_x = cells per tile along x.
+template <class R>
+bool make_push_tensor_map(const Grid<R>& g, int order, int tile_x, int stage_mode, Ctx& c);
 
 // ---- tile_kernels.cu: the tile kernels of one species (needs tile_start): k_push_tile + k_deposit_tile /
 // k_deposit_mma, or k_fused_mma (mode = kDepositTile / kDepositTileMma / kDepositFused); particles they

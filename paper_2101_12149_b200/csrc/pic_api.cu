@@ -206,6 +206,7 @@ struct Sim : SimBase {
     for (int c = 0; c < 6; ++c) g.F[c] = base + (size_t)tot * c;
     for (int c = 0; c < 3; ++c) g.J[c] = base + (size_t)tot * (6 + c);
     PIC_CUDA(cudaMemsetAsync(base, 0, (size_t)tot * 9 * sizeof(R), ctx.stream));
+    make_push_tensor_map<R>(g, order, tile.T[0], o.box_staging, ctx);
     g.Jfix[0] = g.Jfix[1] = nullptr;
     g.fix_scale[0] = g.fix_scale[1] = g.fix_inv[0] = g.fix_inv[1] = 0.0;
     if (deterministic) {
@@ -714,6 +715,7 @@ void pic_default_options(pic_options* o) {
   o->solver = PIC_SOLVER_YEE;
   o->deterministic = 0;
   o->cuda_graph = 1;
+  o->box_staging = PIC_STAGE_AUTO;
   o->cuda_stream = nullptr;
 }
 
@@ -732,7 +734,7 @@ int pic_create(const int32_t n_cells[3], const double dx[3], double dt, int shap
   if (o.sort_interval < 0 || o.sort_key_mode < 0 || o.sort_key_mode > 1 || o.deposit_mode < 0 ||
       o.deposit_mode > 5 || o.pusher < 0 || o.pusher > 1 || o.gather_mode < 0 || o.gather_mode > 1 ||
       o.solver < 0 || o.solver > 1 || o.deterministic < 0 || o.deterministic > 1 ||
-      o.cuda_graph < 0 || o.cuda_graph > 1)
+      o.cuda_graph < 0 || o.cuda_graph > 1 || o.box_staging < 0 || o.box_staging > 2)
     return bad(PIC_ERR_INVALID_ARG, "bad option value");
   double s2 = 0;
   for (int d = 0; d < 3; ++d) {

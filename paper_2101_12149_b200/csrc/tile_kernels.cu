@@ -16,6 +16,7 @@
 // (particles.cu); correctness never depends on the order or the tile.
 #include <algorithm>
 #include <climits>
+#include <type_traits>
 
 #include "internal.h"
 #include "particle_math.cuh"
@@ -48,25 +49,45 @@ __device__ __forceinline__ void tile_coords(const TileSpec& ts, int tile, int* t
 
 // =================================================================== gather + push from shared memory
 // Box of nodes staged per component: local index 0 is node (tile base - HB); EXT nodes per axis cover
-// the stencils (nodal and staggered) of every particle whose cell is inside the tile. Layout: y
-// fastest, then z (stride EXT), x slowest with stride SX = the first value >= EXT^2 that is 9 mod 16.
-// The lanes of a warp hold particles of a few cells that are neighbours along x, so their stencil
-// addresses differ by small multiples of SX (+-1 or +-EXT for a staggered base): with SX = 9 mod 16
-// no two of those fall in the same pair of banks (2.09 wavefronts per 64-bit load, 2.0 is the floor;
-// x fastest gives 2.58), and SX odd keeps the staging stores of an x-row conflict-free.
-template <int ORDER>
+// the stencils (nodal and staggered) of every particle whose cell is inside the tile. Two layouts:
+//  * TMA = false (element-wise cp.async): y fastest, then z (stride EXT), x slowest with stride SX = the
+//    first value >= EXT^2 that is 9 mod 16. The lanes of a warp hold particles of a few cells that are
+//    neighbours along x, so their stencil addresses differ by small multiples of SX (+-1 or +-EXT for a
+//    staggered base): with SX = 9 mod 16 no two of those fall in the same pair of banks (2.10 wavefronts
+//    per 64-bit load at 8 particles per cell, 2.0 is the floor), and SX odd keeps the staging stores of an
+//    x-row conflict-free.
+//  * TMA = true (one cp.async.bulk.tensor per CTA): the copy engine writes the box densely with the
+//    array's fastest axis first, so x is fastest here; the bank spread comes from the box extents
+//    instead: BX x BY x EXT nodes with BX = EXT rounded up to even (the 16-byte rule of the inner box
+//    extent) and BY chosen so that the strides (1, BX, BX*BY) send the same lane patterns to distinct
+//    bank pairs — 12 x 14 x 12 at order 3 gives 2.06 wavefronts per load (12 x 12 x 12 would give 3.04);
+//    the BY - EXT extra rows are loaded and never read.
+template <int ORDER, bool TMA = false, int ES = 8>   // ES = bytes per element
 struct PushBox {
   static constexpr int HB = ORDER == 3 ? 2 : 1;
   static constexpr int EXT = kTileMax + (ORDER == 1 ? 2 : (ORDER == 2 ? 3 : 4));   // 10, 11, 12
   static constexpr int SX = EXT * EXT + ((9 - EXT * EXT % 16) + 16) % 16;            // 105, 121, 153
-  static constexpr int VOL = EXT * SX;
+  // TMA: the copy must start at a 16-byte aligned address, i.e. at an x index of the padded array that is a
+  // multiple of 16 / ES: with tiles that are such a multiple the box starts HBX = 16 / ES nodes below the
+  // tile at every order (XOFF unused x columns where the stencils reach less far down) — a start that is
+  // not aligned raises "illegal instruction" at run time. BX: >= EXT + XOFF, a multiple of 16 / ES.
+  // BY from the bank simulation (fp64: 16 bank pairs, half a warp per wavefront; fp32: 32 banks, a warp).
+  static constexpr int HBX = 16 / ES;                                                // 2 (fp64), 4 (fp32)
+  static constexpr int XOFF = TMA ? HBX - HB : 0;                                    // local x of node (tile base - HB)
+  static constexpr int BX = ES == 8 ? 12 : 16;
+  static constexpr int BY = ES == 8 ? (ORDER == 1 ? 10 : 14) : (ORDER == 3 ? 13 : 11);
+  static constexpr int SA = TMA ? 1 : SX;         // strides (elements) of a step along x, y, z
+  static constexpr int SB = TMA ? BX : 1;
+  static constexpr int SC = TMA ? BX * BY : EXT;
+  static constexpr int VOL = TMA ? BX * BY * EXT : EXT * SX;
   static constexpr int MAXD = 256;   // drifted particles a CTA lists before it gathers them in line
 };
 
 // NX, NY, NZ weights per axis: ORDER + 1, or ORDER along a staggered axis of the Galerkin gather
-template <class R, int ORDER, int NX = ORDER + 1, int NY = ORDER + 1, int NZ = ORDER + 1>
+template <class R, int ORDER, bool TMA, int NX = ORDER + 1, int NY = ORDER + 1, int NZ = ORDER + 1>
 __device__ __forceinline__ R interp_box(const R* __restrict__ F, int base, const R* wx, const R* wy, const R* wz) {
-  constexpr int E = PushBox<ORDER>::EXT, SX = PushBox<ORDER>::SX;
+  using PB = PushBox<ORDER, TMA, (int)sizeof(R)>;
+  constexpr int SA = PB::SA, SB = PB::SB, SC = PB::SC;
   R acc = 0;
   if constexpr (kStatementOrder<R>) {   // sum over c, b, a (a innermost) of ((wx wy) wz) F, every operation rounded
 #pragma unroll
@@ -75,7 +96,7 @@ __device__ __forceinline__ R interp_box(const R* __restrict__ F, int base, const
       for (int b = 0; b < NY; ++b)
 #pragma unroll
         for (int a = 0; a < NX; ++a)
-          acc = add_rn(acc, mul_rn(mul_rn(mul_rn(wx[a], wy[b]), wz[c]), F[base + SX * a + b + E * c]));
+          acc = add_rn(acc, mul_rn(mul_rn(mul_rn(wx[a], wy[b]), wz[c]), F[base + SA * a + SB * b + SC * c]));
   } else {
 #pragma unroll
     for (int c = 0; c < NZ; ++c) {
@@ -84,13 +105,45 @@ __device__ __forceinline__ R interp_box(const R* __restrict__ F, int base, const
       for (int b = 0; b < NY; ++b) {
         R acca = 0;
 #pragma unroll
-        for (int a = 0; a < NX; ++a) acca += wx[a] * F[base + SX * a + b + E * c];
+        for (int a = 0; a < NX; ++a) acca += wx[a] * F[base + SA * a + SB * b + SC * c];
         accb += wy[b] * acca;
       }
       acc += wz[c] * accb;
     }
   }
   return acc;
+}
+
+// ---- TMA + mbarrier primitives (sm_90+ PTX; SASS: UTMALDG, SYNCS)
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(bar);
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}" ::"r"(a), "r"(parity)
+      : "memory");
+}
+// one 4-D tile (x, y, z, component) of the tensor `tmap` describes -> shared memory, completion on `bar`;
+// coordinates may start below 0 or end past the tensor: those elements arrive as zeros
+__device__ __forceinline__ void tma_load_4d(void* smem_dst, const CUtensorMap* tmap, unsigned long long* bar, int c0, int c1,
+                                            int c2, int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];" ::"r"(
+          (unsigned)__cvta_generic_to_shared(smem_dst)),
+      "l"(tmap), "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3)
+      : "memory");
 }
 
 template <class R, int PUSHER>
@@ -108,18 +161,24 @@ __device__ __forceinline__ void push_store(const Grid<R>& g, const Particles<R>&
 // per order and precision, (0, 0) being the default and benchmarked path. The Galerkin gather carries one
 // weight less along every staggered axis, so it reads 288 box elements per particle instead of 384 at
 // order 3 — and runs faster by that ratio, since those reads are what bounds the kernel.
-template <class R, int ORDER, int PUSHER, int GATHER>
+// TMA: the box arrives by ONE bulk tensor copy issued by one thread (all six components: the field arrays
+// are one allocation, described as a 4-D tensor), signalled on an mbarrier; meanwhile every thread already
+// loads its first particle. Otherwise 6 * EXT^3 element-wise cp.async copies.
+template <class R, int ORDER, int PUSHER, int GATHER, bool TMA>
 __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn,
                                                                    R* __restrict__ yn, R* __restrict__ zn,
-                                                                   const int32_t* __restrict__ tile_start, TileSpec ts) {
-  using PB = PushBox<ORDER>;
-  constexpr int E = PB::EXT, SX = PB::SX, VOL = PB::VOL;
+                                                                   const int32_t* __restrict__ tile_start, TileSpec ts,
+                                                                   const __grid_constant__ CUtensorMap tmap) {
+  using PB = PushBox<ORDER, TMA, (int)sizeof(R)>;
+  constexpr int E = PB::EXT, VOL = PB::VOL, SA = PB::SA, SB = PB::SB, SC = PB::SC;
   constexpr int NS = GATHER == 1 ? ORDER : ORDER + 1;   // weights along a staggered axis
   constexpr int NN = ORDER + 1;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  R* box = reinterpret_cast<R*>(smem_raw);   // [6][E (x)][SX: E (z) x E (y), padded]
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  R* box_raw = reinterpret_cast<R*>(smem_raw);   // [6][VOL]
+  R* box = box_raw + PB::XOFF * SA;              // local (0,0,0) = node (tile base - HB)
   __shared__ int s_drift[PB::MAXD];
   __shared__ int s_ndrift;
+  __shared__ __align__(8) unsigned long long s_bar;
   const int tile = blockIdx.x;
   const int s = tile_start[tile], e = tile_start[tile + 1];
   if (s >= e) return;
@@ -127,24 +186,37 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
   int tb[3];
   tile_coords(ts, tile, tb);
   const int o0 = tb[0] - PB::HB, o1 = tb[1] - PB::HB, o2 = tb[2] - PB::HB;   // node of local (0,0,0)
-  // stage the six boxes, reading along x (nodes beyond the padded array, possible only for tiles
-  // smaller than 8, read 0)
-  const int lim0 = g.N[0] + kGuard, lim1 = g.N[1] + kGuard, lim2 = g.N[2] + kGuard;
-  for (int idx = threadIdx.x; idx < E * E * E; idx += blockDim.x) {
-    int i = idx % E, r = idx / E;
-    int j = r % E, k = r / E;
-    const bool in = (o0 + i < lim0) & (o1 + j < lim1) & (o2 + k < lim2);
-    const int gi = g.idx(o0 + i, o1 + j, o2 + k);
-    const int li = SX * i + j + E * k;
-    // asynchronous copies (LDGSTS): every element of the box is in flight at once, no register staging
+  if constexpr (TMA) {
+    if (threadIdx.x == 0) {
+      mbar_init(&s_bar, 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+      mbar_expect_tx(&s_bar, (unsigned)(6 * VOL * sizeof(R)));
+      tma_load_4d(box_raw, &tmap, &s_bar, tb[0] - PB::HBX + kGuard, o1 + kGuard, o2 + kGuard, 0);
+    }
+    __syncthreads();   // the barrier object (and s_ndrift) visible to every thread before anyone waits on it
+  } else {
+    // stage the six boxes, reading along x (nodes beyond the padded array, possible only for tiles
+    // smaller than 8, read 0)
+    const int lim0 = g.N[0] + kGuard, lim1 = g.N[1] + kGuard, lim2 = g.N[2] + kGuard;
+    for (int idx = threadIdx.x; idx < E * E * E; idx += blockDim.x) {
+      int i = idx % E, r = idx / E;
+      int j = r % E, k = r / E;
+      const bool in = (o0 + i < lim0) & (o1 + j < lim1) & (o2 + k < lim2);
+      const int gi = g.idx(o0 + i, o1 + j, o2 + k);
+      const int li = SA * i + SB * j + SC * k;
+      // asynchronous copies (LDGSTS): every element of the box is in flight at once, no register staging
 #pragma unroll
-    for (int c = 0; c < 6; ++c) {
-      if (in) cp_async(box + c * VOL + li, g.F[c] + gi);
-      else box[c * VOL + li] = R(0);
+      for (int c = 0; c < 6; ++c) {
+        if (in) cp_async(box + c * VOL + li, g.F[c] + gi);
+        else box[c * VOL + li] = R(0);
+      }
     }
   }
-  asm volatile("cp.async.wait_all;" ::: "memory");
-  __syncthreads();
+  bool staged = !TMA;
+  if constexpr (!TMA) {
+    asm volatile("cp.async.wait_all;" ::: "memory");
+    __syncthreads();
+  }
   for (int t = s + threadIdx.x; t < e; t += blockDim.x) {
     R x0[3] = {p.x[t], p.y[t], p.z[t]};
     R u[3] = {p.ux[t], p.uy[t], p.uz[t]};
@@ -165,31 +237,52 @@ __global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Pa
               (d == 0 ? o0 : (d == 1 ? o1 : o2));
       inbox &= (ln[d] >= 0) & (ln[d] <= E - ORDER - 1) & (ls[d] >= 0) & (ls[d] <= E - ORDER - 1);
     }
+    if constexpr (TMA) {
+      if (!staged) {   // the box has been on its way while the first particle was loaded and its weights formed
+        mbar_wait(&s_bar, 0);
+        staged = true;
+      }
+    }
     if (!inbox) {
-      // drifted out of the tile since the last sort: listed, gathered from global memory below with
-      // all lanes busy (in line if the list is full)
+      // drifted out of the tile since the last sort: listed, gathered from global memory below with all
+      // lanes busy. If the list overflows the entry is dropped and the second pass finds these particles by
+      // walking the tile again: ONE copy of the global-memory gather, so that a particle's result never
+      // depends on which threads reached the list first (bit-identical runs, pic_options.deterministic)
       const int slot = atomicAdd(&s_ndrift, 1);
-      if (slot < PB::MAXD) { s_drift[slot] = t; continue; }
-      R Ef[3], Bf[3];
-      gather6<R, ORDER, GATHER != 0>(g, x0[0], x0[1], x0[2], Ef, Bf);
-      push_store<R, PUSHER>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
+      if (slot < PB::MAXD) s_drift[slot] = t;
       continue;
     }
     R Ef[3], Bf[3];
     // Ex (s,n,n)  Ey (n,s,n)  Ez (n,n,s)  Bx (n,s,s)  By (s,n,s)  Bz (s,s,n)
-    Ef[0] = interp_box<R, ORDER, NS, NN, NN>(box + 0 * VOL, SX * ls[0] + ln[1] + E * ln[2], ws[0], wn[1], wn[2]);
-    Ef[1] = interp_box<R, ORDER, NN, NS, NN>(box + 1 * VOL, SX * ln[0] + ls[1] + E * ln[2], wn[0], ws[1], wn[2]);
-    Ef[2] = interp_box<R, ORDER, NN, NN, NS>(box + 2 * VOL, SX * ln[0] + ln[1] + E * ls[2], wn[0], wn[1], ws[2]);
-    Bf[0] = interp_box<R, ORDER, NN, NS, NS>(box + 3 * VOL, SX * ln[0] + ls[1] + E * ls[2], wn[0], ws[1], ws[2]);
-    Bf[1] = interp_box<R, ORDER, NS, NN, NS>(box + 4 * VOL, SX * ls[0] + ln[1] + E * ls[2], ws[0], wn[1], ws[2]);
-    Bf[2] = interp_box<R, ORDER, NS, NS, NN>(box + 5 * VOL, SX * ls[0] + ls[1] + E * ln[2], ws[0], ws[1], wn[2]);
+    Ef[0] = interp_box<R, ORDER, TMA, NS, NN, NN>(box + 0 * VOL, SA * ls[0] + SB * ln[1] + SC * ln[2], ws[0], wn[1], wn[2]);
+    Ef[1] = interp_box<R, ORDER, TMA, NN, NS, NN>(box + 1 * VOL, SA * ln[0] + SB * ls[1] + SC * ln[2], wn[0], ws[1], wn[2]);
+    Ef[2] = interp_box<R, ORDER, TMA, NN, NN, NS>(box + 2 * VOL, SA * ln[0] + SB * ln[1] + SC * ls[2], wn[0], wn[1], ws[2]);
+    Bf[0] = interp_box<R, ORDER, TMA, NN, NS, NS>(box + 3 * VOL, SA * ln[0] + SB * ls[1] + SC * ls[2], wn[0], ws[1], ws[2]);
+    Bf[1] = interp_box<R, ORDER, TMA, NS, NN, NS>(box + 4 * VOL, SA * ls[0] + SB * ln[1] + SC * ls[2], ws[0], wn[1], ws[2]);
+    Bf[2] = interp_box<R, ORDER, TMA, NS, NS, NN>(box + 5 * VOL, SA * ls[0] + SB * ls[1] + SC * ln[2], ws[0], ws[1], wn[2]);
     push_store<R, PUSHER>(g, p, xn, yn, zn, t, x0, u, Ef, Bf);
   }
   __syncthreads();
-  const int nd = min(s_ndrift, PB::MAXD);
-  for (int q = threadIdx.x; q < nd; q += blockDim.x) {
-    const int t = s_drift[q];
+  const int nd = s_ndrift;
+  const bool rescan = nd > PB::MAXD;   // warp-uniform (CTA-uniform)
+  const int cnt = rescan ? e - s : nd;
+  for (int q = threadIdx.x; q < cnt; q += blockDim.x) {
+    const int t = rescan ? s + q : s_drift[q];
     R x0[3] = {p.x[t], p.y[t], p.z[t]};
+    if (rescan) {   // the same test as above, on the same bits
+      bool inbox = true;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) {
+        R wtmp[ORDER + 1];
+        const R xi = mul_rn(x0[d], g.inv_dx[d]);
+        const R xs = sub_rn(xi, R(0.5));
+        const int od = d == 0 ? o0 : (d == 1 ? o1 : o2);
+        const int l_n = shape<R, ORDER>(xi, wtmp) - od;
+        const int l_s = (GATHER == 1 ? shape_lowered<R, ORDER>(xs, wtmp) : shape<R, ORDER>(xs, wtmp)) - od;
+        inbox &= (l_n >= 0) & (l_n <= E - ORDER - 1) & (l_s >= 0) & (l_s <= E - ORDER - 1);
+      }
+      if (inbox) continue;
+    }
     R u[3] = {p.ux[t], p.uy[t], p.uz[t]};
     R Ef[3], Bf[3];
     gather6<R, ORDER, GATHER != 0>(g, x0[0], x0[1], x0[2], Ef, Bf);
@@ -301,23 +394,23 @@ __device__ __forceinline__ void axis_window_ext(R xi0, R xi1, int& cell, R* S0, 
     }
     ext = sh == 0 ? 0 : (sh == -1 ? 1 : (sh == 1 ? 2 : 3));
     dext = sh < 0 ? w1[0] : w1[ORDER];
-    return;
-  }
+  } else {
 #pragma unroll
-  for (int i = 0; i < NW; ++i) {
-    R a = 0, b = 0;
+    for (int i = 0; i < NW; ++i) {
+      R a = 0, b = 0;
 #pragma unroll
-    for (int k = 0; k <= ORDER; ++k) {
-      a = (i == so0 + k) ? w0[k] : a;
-      b = (i == sl1 + k) ? w1[k] : b;
+      for (int k = 0; k <= ORDER; ++k) {
+        a = (i == so0 + k) ? w0[k] : a;
+        b = (i == sl1 + k) ? w1[k] : b;
+      }
+      S0[i] = a;
+      DS[i] = sub_rn(b, a);
     }
-    S0[i] = a;
-    DS[i] = sub_rn(b, a);
+    const bool oldfits = (so0 >= 0) & (so0 + ORDER < NW);
+    const bool fits = (sl1 >= 0) & (sl1 + ORDER < NW);
+    ext = !oldfits ? 3 : (fits ? 0 : (sl1 == -1 ? 1 : (sl1 + ORDER == NW ? 2 : 3)));
+    dext = sl1 < 0 ? w1[0] : w1[ORDER];
   }
-  const bool oldfits = (so0 >= 0) & (so0 + ORDER < NW);
-  const bool fits = (sl1 >= 0) & (sl1 + ORDER < NW);
-  ext = !oldfits ? 3 : (fits ? 0 : (sl1 == -1 ? 1 : (sl1 + ORDER == NW ? 2 : 3)));
-  dext = sl1 < 0 ? w1[0] : w1[ORDER];
 }
 
 // The extra node of the particles of a round that crossed a face in y or in z (axis_window_ext): for each
@@ -526,7 +619,7 @@ __global__ void __launch_bounds__(NWARP * 32, 2)
   using W = TWin<ORDER>;
   constexpr int NX = W::NX, NYZ = W::NYZ, LG = W::LG, REC = W::REC;
   constexpr bool kExt = ORDER != 1;   // extra node of a face crossing in y or z taken here (see below)
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   R* rec_all = reinterpret_cast<R*>(smem_raw);
   __shared__ int s_order[NWARP][32];
 
@@ -721,7 +814,7 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
                   unsigned int* __restrict__ stray_count, unsigned long long* deactivated) {
   using W = MWin<ORDER>;
   constexpr int NX = W::NX, NYZ = W::NYZ, NB = W::NB, REC = W::REC, BLX = W::BLX, BLYZ = W::BLYZ;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   R* rec_all = reinterpret_cast<R*>(smem_raw);
 
   const int tile = blockIdx.x;
@@ -920,7 +1013,7 @@ __global__ void __launch_bounds__(NWARP * 32, 1)
   constexpr int NN = ORDER + 1;
   constexpr int NX = W::NX, NYZ = W::NYZ, NB = W::NB, REC = W::REC, BLX = W::BLX, BLYZ = W::BLYZ;
   constexpr int MAXD = kFusedMaxDrift;
-  extern __shared__ __align__(16) unsigned char smem_raw[];
+  extern __shared__ __align__(128) unsigned char smem_raw[];
   R* box = reinterpret_cast<R*>(smem_raw);   // [6][E (x)][SX: E (z) x E (y), padded]
   R* rec_all = box + 6 * VOL;
   __shared__ int s_drift[NWARP][MAXD];   // per warp, in processing order: nothing here depends on timing
@@ -1053,12 +1146,12 @@ __global__ void __launch_bounds__(NWARP * 32, 1)
           if (inbox) {
             const int l0 = ln[0] - o0, l1 = ln[1] - o1, l2 = ln[2] - o2;
             // Ex (s,n,n)  Ey (n,s,n)  Ez (n,n,s)  Bx (n,s,s)  By (s,n,s)  Bz (s,s,n)
-            Ef[0] = interp_box<R, ORDER, NS, NN, NN>(box + 0 * VOL, SX * ls[0] + l1 + E * l2, ws[0], wn[1], wn[2]);
-            Ef[1] = interp_box<R, ORDER, NN, NS, NN>(box + 1 * VOL, SX * l0 + ls[1] + E * l2, wn[0], ws[1], wn[2]);
-            Ef[2] = interp_box<R, ORDER, NN, NN, NS>(box + 2 * VOL, SX * l0 + l1 + E * ls[2], wn[0], wn[1], ws[2]);
-            Bf[0] = interp_box<R, ORDER, NN, NS, NS>(box + 3 * VOL, SX * l0 + ls[1] + E * ls[2], wn[0], ws[1], ws[2]);
-            Bf[1] = interp_box<R, ORDER, NS, NN, NS>(box + 4 * VOL, SX * ls[0] + l1 + E * ls[2], ws[0], wn[1], ws[2]);
-            Bf[2] = interp_box<R, ORDER, NS, NS, NN>(box + 5 * VOL, SX * ls[0] + ls[1] + E * l2, ws[0], ws[1], wn[2]);
+            Ef[0] = interp_box<R, ORDER, false, NS, NN, NN>(box + 0 * VOL, SX * ls[0] + l1 + E * l2, ws[0], wn[1], wn[2]);
+            Ef[1] = interp_box<R, ORDER, false, NN, NS, NN>(box + 1 * VOL, SX * l0 + ls[1] + E * l2, wn[0], ws[1], wn[2]);
+            Ef[2] = interp_box<R, ORDER, false, NN, NN, NS>(box + 2 * VOL, SX * l0 + l1 + E * ls[2], wn[0], wn[1], ws[2]);
+            Bf[0] = interp_box<R, ORDER, false, NN, NS, NS>(box + 3 * VOL, SX * l0 + ls[1] + E * ls[2], wn[0], ws[1], ws[2]);
+            Bf[1] = interp_box<R, ORDER, false, NS, NN, NS>(box + 4 * VOL, SX * ls[0] + l1 + E * ls[2], ws[0], wn[1], ws[2]);
+            Bf[2] = interp_box<R, ORDER, false, NS, NS, NN>(box + 5 * VOL, SX * ls[0] + ls[1] + E * l2, ws[0], ws[1], wn[2]);
           }
         }
         drifted = !inbox;
@@ -1225,15 +1318,21 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, int mo
   auto kvec = det ? k_deposit_tile<R, ORDER, kW, 1> : k_deposit_tile<R, ORDER, kW, 0>;
   auto kmma = det ? k_deposit_mma<R, ORDER, kDepMmaWarps, kDepMmaCtas, 1> : k_deposit_mma<R, ORDER, kDepMmaWarps, kDepMmaCtas, 0>;
   constexpr int mw = kDepMmaWarps;
-  const size_t push_smem = (size_t)6 * PushBox<ORDER>::VOL * sizeof(R);
+  const bool tma = c.tma_push;
+  constexpr int ES = (int)sizeof(R);
+  const size_t push_smem = (size_t)6 * (tma ? PushBox<ORDER, true, ES>::VOL : PushBox<ORDER, false, ES>::VOL) * sizeof(R);
   const size_t vec_smem = (size_t)kW * 32 * TWin<ORDER>::REC * sizeof(R);
   const size_t mma_smem = (size_t)mw * 33 * MWin<ORDER>::REC * sizeof(R);
   {
     ScopedPhase ph(c, kPhasePush);
-    auto kpush = g.pusher == 0 ? (g.gather_mode == 0 ? k_push_tile<R, ORDER, 0, 0> : k_push_tile<R, ORDER, 0, 1>)
-                               : (g.gather_mode == 0 ? k_push_tile<R, ORDER, 1, 0> : k_push_tile<R, ORDER, 1, 1>);
+    auto pick = [&](auto tma_tag) {
+      constexpr bool T = decltype(tma_tag)::value;
+      return g.pusher == 0 ? (g.gather_mode == 0 ? k_push_tile<R, ORDER, 0, 0, T> : k_push_tile<R, ORDER, 0, 1, T>)
+                           : (g.gather_mode == 0 ? k_push_tile<R, ORDER, 1, 0, T> : k_push_tile<R, ORDER, 1, 1, T>);
+    };
+    auto kpush = tma ? pick(std::true_type{}) : pick(std::false_type{});
     opt_in_smem(c, kpush, push_smem);
-    kpush<<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles);
+    kpush<<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, c.tmap_push);
   }
   {
     ScopedPhase ph(c, kPhaseDeposit);
@@ -1249,6 +1348,51 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, int mo
   }
   c.launches += 2;
 }
+
+// The six E/B arrays are one allocation of six padded boxes (pic_api.cu), i.e. a 4-D tensor (x, y, z,
+// component) with x contiguous. TMA needs every stride to be a multiple of 16 bytes and the base 16-byte
+// aligned; grids that do not meet that (odd padded extents, odd tiles) keep the cp.async staging.
+template <class R>
+bool make_push_tensor_map(const Grid<R>& g, int order, int tile_x, int stage_mode, Ctx& c) {
+  c.tma_push = false;
+  if (stage_mode == 1) return false;                       // PIC_STAGE_CP_ASYNC
+  if ((tile_x * sizeof(R)) % 16) return false;             // every box must start at a 16-byte aligned x
+  const size_t es = sizeof(R);
+  const size_t st1 = (size_t)g.P[0] * es, st2 = st1 * g.P[1], st3 = st2 * g.P[2];
+  if (st1 % 16 || st2 % 16 || st3 % 16 || ((uintptr_t)g.F[0] % 16)) return false;
+  for (int k = 1; k < 6; ++k)
+    if (g.F[k] != g.F[0] + (size_t)k * (st3 / es)) return false;
+  typedef CUresult (*EncodeFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                               const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                               CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn ||
+      qres != cudaDriverEntryPointSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  constexpr int ES = (int)sizeof(R);
+  cuuint32_t box[4];
+  switch (order) {
+    case 1: box[0] = PushBox<1, true, ES>::BX; box[1] = PushBox<1, true, ES>::BY; box[2] = PushBox<1, true, ES>::EXT; break;
+    case 2: box[0] = PushBox<2, true, ES>::BX; box[1] = PushBox<2, true, ES>::BY; box[2] = PushBox<2, true, ES>::EXT; break;
+    default: box[0] = PushBox<3, true, ES>::BX; box[1] = PushBox<3, true, ES>::BY; box[2] = PushBox<3, true, ES>::EXT; break;
+  }
+  box[3] = 6;
+  if ((box[0] * es) % 16) return false;
+  const cuuint64_t dims[4] = {(cuuint64_t)g.P[0], (cuuint64_t)g.P[1], (cuuint64_t)g.P[2], 6};
+  const cuuint64_t strides[3] = {st1, st2, st3};
+  const cuuint32_t estr[4] = {1, 1, 1, 1};
+  const CUresult r = ((EncodeFn)fn)(&c.tmap_push, es == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 4,
+                                    (void*)g.F[0], dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                    CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  c.tma_push = r == CUDA_SUCCESS;
+  return c.tma_push;
+}
+template bool make_push_tensor_map<double>(const Grid<double>&, int, int, int, Ctx&);
+template bool make_push_tensor_map<float>(const Grid<float>&, int, int, int, Ctx&);
 
 template <class R>
 void launch_tile_kernels(const Grid<R>& g, const ParticleStep<R>& a, int order, int mode, Ctx& c) {
