@@ -816,6 +816,7 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
   constexpr int NX = W::NX, NYZ = W::NYZ, NB = W::NB, REC = W::REC, BLX = W::BLX, BLYZ = W::BLYZ;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   R* rec_all = reinterpret_cast<R*>(smem_raw);
+  __shared__ unsigned char s_ord[NWARP][32];   // record slots of the group being contracted, in order
 
   const int tile = blockIdx.x;
   const int s = tile_start[tile], e = tile_start[tile + 1];
@@ -912,35 +913,40 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
       }
     }
     __syncwarp();
-    // runs of consecutive particles whose cells lie in the same triple of x-neighbouring cells of one
+    // groups of particles of this round whose cells lie in the same triple of x-neighbouring cells of one
     // (y,z) row: their windows span 8 nodes together, exactly the 8 rows of C, so they share the
-    // accumulators (fewer padded contraction steps, and three rows retire at once). The order is
-    // cell-sorted up to drift since the last sort; a triple met twice is simply accumulated twice.
-    // Warp-uniform control flow.
+    // accumulators (fewer padded contraction steps, and three rows retire at once). The groups are formed
+    // over the whole round, not over consecutive particles: in a hot plasma the order is stale between two
+    // sorts, and every particle out of place would otherwise end a run and send the accumulated rows to J
+    // (C5: L2 at 69 % with reductions). The triple being accumulated goes first. Warp-uniform control flow.
     const int scode = code < 0 ? -1 : ((code & ~15) | ((code & 15) / 3));
-    const int prev = __shfl_up_sync(0xffffffffu, scode, 1);
-    unsigned heads = __ballot_sync(0xffffffffu, lane == 0 || scode != prev);
-    const unsigned live = __ballot_sync(0xffffffffu, code >= 0);
-    while (heads) {
-      const int s0 = __ffs(heads) - 1;
-      heads &= heads - 1;
-      const int s1 = heads ? __ffs(heads) - 1 : 32;
-      if (!((live >> s0) & 1u)) continue;
-      const int cd = __shfl_sync(0xffffffffu, scode, s0);
+    unsigned rem = __ballot_sync(0xffffffffu, code >= 0);
+    while (rem) {
+      unsigned m = cur != INT_MIN ? (__ballot_sync(0xffffffffu, scode == cur) & rem) : 0u;
+      int cd = cur;
+      if (m == 0) {
+        cd = __shfl_sync(0xffffffffu, scode, __ffs(rem) - 1);
+        m = __ballot_sync(0xffffffffu, scode == cd);
+      }
+      rem &= ~m;
+      if ((m >> lane) & 1u) s_ord[warp][__popc(m & ((1u << lane) - 1u))] = (unsigned char)lane;
+      __syncwarp();
+      const int cnt = __popc(m);
       if (cd != cur) {
         if (cur != INT_MIN) retire_rows(((cd ^ cur) >> 4) == 0, win_x(cd));
         cur = cd;
       }
 #pragma unroll 2
-      for (int b = s0; b < s1; b += 4) {
-        // four particles per contraction step, K = particle: this lane supplies, for particle b + t,
-        // the A operands of its row (a node of that particle's own 6-node window, or zero) and the
+      for (int b = 0; b < cnt; b += 4) {
+        // four particles per contraction step, K = particle: this lane supplies, for the group's particle
+        // b + t, the A operands of its row (a node of that particle's own 6-node window, or zero) and the
         // B operands of its column(s)
-        const bool here = b + t < s1;
-        const int pc = __shfl_sync(0xffffffffu, code, (b + t) & 31);
+        const bool here = b + t < cnt;
+        const int src = here ? (int)s_ord[warp][b + t] : 32;          // slot 32: the all-zero record
+        const int pc = __shfl_sync(0xffffffffu, code, src & 31);
         const int i = (gq - (tb[0] + (pc & 15) - 4 - BLX)) & 7;      // window slot of this lane's row
         const bool rowok = i < NX;
-        const R* rr = rec + (here ? b + t : 32) * REC;               // slot 32: the all-zero record
+        const R* rr = rec + src * REC;
         const R* ra = rowok ? rr : zrec;
         const double px = ra[W::oPX + (rowok ? i : 0)];
         const Pair2<R> ab = *reinterpret_cast<const Pair2<R>*>(ra + W::oAB + 2 * (rowok ? i : 0));
@@ -960,6 +966,7 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
           dmma_884(C.z[nb][0], C.z[nb][1], (double)ab.b, pz * y1);
         }
       }
+      __syncwarp();   // s_ord is rewritten by the next group
     }
     extra_node_deposit<R, ORDER, DET, W>(g, rec, extc, x1[1], x1[2], w, p.jf, tb[0] + (code & 15) - 4 - BLX,
                                          tb[1] + ((code >> 4) & 15) - 4 - BLYZ, tb[2] + (code >> 8) - 4 - BLYZ);
@@ -1357,6 +1364,9 @@ bool make_push_tensor_map(const Grid<R>& g, int order, int tile_x, int stage_mod
   c.tma_push = false;
   if (stage_mode == 1) return false;                       // PIC_STAGE_CP_ASYNC
   if ((tile_x * sizeof(R)) % 16) return false;             // every box must start at a 16-byte aligned x
+  // fp32: only on request. Measured on C3 (order 1): push 0.405 ms with TMA against 0.396 ms with cp.async —
+  // the box is small (10^3 nodes of 4 bytes) and the y-fastest layout has slightly fewer bank conflicts there.
+  if (sizeof(R) != 8 && stage_mode != 2) return false;
   const size_t es = sizeof(R);
   const size_t st1 = (size_t)g.P[0] * es, st2 = st1 * g.P[1], st3 = st2 * g.P[2];
   if (st1 % 16 || st2 % 16 || st3 % 16 || ((uintptr_t)g.F[0] % 16)) return false;
