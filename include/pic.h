@@ -149,6 +149,8 @@ PIC_API void pic_default_options(pic_options* opt);
 /* Create a simulation on the current CUDA device: a box of n_cells[3] Yee cells of size dx[3]
  * (metres), time step dt (seconds), B-spline shape order 1..3 used for both gather and deposit,
  * working precision prec. Fields start at zero. *out receives the handle.
+ * Limits: field nodes are indexed with 32 bits, (n_cells + 8)^3 padded nodes must stay below 2^31
+ * (INVALID_ARG otherwise), and the sort key (tiles x cells per tile) below 2^32.
  * Errors: INVALID_ARG, CFL, OOM, CUDA. */
 PIC_API int pic_create(const int32_t n_cells[3], const double dx[3], double dt, int shape_order,
                pic_precision prec, const pic_options* opt, pic_sim** out);
@@ -157,6 +159,8 @@ PIC_API int pic_create(const int32_t n_cells[3], const double dx[3], double dt, 
  * and mass (kg) per real particle. x..w are arrays of n elements in `where` memory. Particle ids
  * are 0..n-1 in the order given and follow the particles through every sort. *species_id
  * (nullable) receives the species index (0,1,...). Species are processed in insertion order.
+ * Limit: particle slots are indexed with 32 bits inside the kernels (tile_start[], the stray list,
+ * perm[]), so n < 2^31 per species (INVALID_ARG otherwise); the number of species is not limited.
  * Errors: INVALID_ARG (incl. non-finite values), OUT_OF_DOMAIN, OOM, CUDA. Synchronises. */
 PIC_API int pic_add_species(pic_sim* sim, int64_t n, const void* x, const void* y, const void* z,
                     const void* ux, const void* uy, const void* uz, const void* w,
