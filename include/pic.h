@@ -146,7 +146,10 @@ typedef struct {
 /* Fill *opt with the defaults. */
 PIC_API void pic_default_options(pic_options* opt);
 
-/* Create a simulation on the current CUDA device: a box of n_cells[3] Yee cells of size dx[3]
+/* A handle belongs to the CUDA device that is current when pic_create is called; every later call on it
+ * makes that device current for its duration and restores the caller's device before returning.
+ *
+ * Create a simulation on the current CUDA device: a box of n_cells[3] Yee cells of size dx[3]
  * (metres), time step dt (seconds), B-spline shape order 1..3 used for both gather and deposit,
  * working precision prec. Fields start at zero. *out receives the handle.
  * Limits: field nodes are indexed with 32 bits, (n_cells + 8)^3 padded nodes must stay below 2^31

@@ -56,6 +56,7 @@ struct SimBase {
   virtual ~SimBase() {}
   std::string err;
   int prec = 0;
+  int device = 0;   // the CUDA device the handle lives on (every ABI call switches to it and back)
   virtual int add_species(int64_t n, const void* const* arr, double q, double m, pic_mem where, int32_t* id) = 0;
   virtual int set_fields(const void* const* E, const void* const* B, pic_mem where) = 0;
   virtual int step(int n) = 0;
@@ -161,6 +162,7 @@ struct Sim : SimBase {
     use_graph = o.cuda_graph != 0;
     ctx.stream = (cudaStream_t)o.cuda_stream;
     PIC_CUDA(cudaGetDevice(&ctx.device));
+    this->device = ctx.device;
     PIC_CUDA(cudaDeviceGetAttribute(&ctx.sm_count, cudaDevAttrMultiProcessorCount, ctx.device));
     int64_t tot = 1;
     for (int d = 0; d < 3; ++d) {
@@ -778,8 +780,22 @@ int pic_create(const int32_t n_cells[3], const double dx[3], double dt, int shap
   return PIC_OK;
 }
 
-#define SIM_OR_FAIL(s) \
-  if (!(s) || !(s)->impl) return PIC_ERR_INVALID_ARG
+// A handle belongs to the device that was current at pic_create: its memory, stream, function attributes
+// and tensor map live there. Every call on a handle makes that device current for its duration and restores
+// the caller's afterwards, so a process that drives several GPUs can hold one handle per device.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() {
+    if (switched) cudaSetDevice(prev);
+  }
+};
+#define SIM_OR_FAIL(s)                               \
+  if (!(s) || !(s)->impl) return PIC_ERR_INVALID_ARG; \
+  DeviceGuard device_guard_((s)->impl->device)
 
 int pic_add_species(pic_sim* sim, int64_t n, const void* x, const void* y, const void* z, const void* ux,
                     const void* uy, const void* uz, const void* w, double charge, double mass, pic_mem where,
@@ -874,6 +890,7 @@ int pic_ckc_coefficients(const double dx[3], double alpha[3], double beta[9], do
 
 void pic_destroy(pic_sim* sim) {
   if (!sim) return;
+  DeviceGuard device_guard_(sim->impl ? sim->impl->device : 0);
   delete sim->impl;
   delete sim;
 }
