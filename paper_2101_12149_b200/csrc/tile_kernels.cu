@@ -936,7 +936,11 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
         if (cur != INT_MIN) retire_rows(((cd ^ cur) >> 4) == 0, win_x(cd));
         cur = cd;
       }
-#pragma unroll 2
+#ifndef PIC_X_UNROLL
+#define PIC_X_UNROLL 2
+#endif
+      constexpr int kUnrollSteps = PIC_X_UNROLL;
+#pragma unroll kUnrollSteps
       for (int b = 0; b < cnt; b += 4) {
         // four particles per contraction step, K = particle: this lane supplies, for the group's particle
         // b + t, the A operands of its row (a node of that particle's own 6-node window, or zero) and the
