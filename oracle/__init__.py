@@ -15,7 +15,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "pic_oracle.cpp")
-_LIB = os.path.join(_HERE, "liboracle.so")
+# ORACLE_SANITIZE=1: an AddressSanitizer + UndefinedBehaviorSanitizer build of the same source, loaded instead
+# (run python with libasan / libubsan preloaded — command in profiles/oracle_sanitizers.md)
+_SANITIZE = os.environ.get("ORACLE_SANITIZE", "") == "1"
+_LIB = os.path.join(_HERE, "liboracle_san.so" if _SANITIZE else "liboracle.so")
 
 DIAG = ("field_E", "field_B", "kinetic", "charge", "gauss_max", "rho_max", "deactivated", "steps")
 
@@ -24,9 +27,10 @@ def build(force: bool = False) -> str:
     """Compile the oracle (g++ -O2 -ffp-contract=off -fopenmp). Returns the library path."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
         tmp = _LIB + ".tmp%d" % os.getpid()
+        extra = ["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] if _SANITIZE else []
         subprocess.check_call(
-            ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC",
-             "-o", tmp, _SRC])
+            ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-shared", "-fPIC"] + extra +
+            ["-o", tmp, _SRC])
         os.replace(tmp, _LIB)
     return _LIB
 

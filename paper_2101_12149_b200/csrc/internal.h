@@ -1,5 +1,6 @@
 // Host-side declarations shared by the translation units of libpic.so (CUDA path only).
 #pragma once
+#include <nvtx3/nvToolsExt.h>   // header-only NVTX v3
 #include <cuda.h>   // CUtensorMap (types only: the encoder is fetched with cudaGetDriverEntryPoint, nothing links libcuda)
 
 #include <set>
@@ -90,14 +91,24 @@ struct Ctx {
   Timer timer;
 };
 
-// times everything launched on c.stream during its lifetime as one span of `phase`
+// times everything launched on c.stream during its lifetime as one span of `phase`, and brackets it with an
+// NVTX range of the phase's name (the host-side launch window of each kernel class shows up
+// in a timeline tool; NVTX v3 is header-only and does nothing when no tool is attached)
+enum { kPhaseSort = 0, kPhasePush = 1, kPhaseDeposit = 2, kPhaseStray = 3, kPhaseFields = 4 };
+inline const char* phase_name(int phase) {
+  static const char* const names[kNumPhases] = {"pic:sort", "pic:gather+push", "pic:deposit", "pic:deposit(per-particle)",
+                                                "pic:fields"};
+  return phase >= 0 && phase < kNumPhases ? names[phase] : "pic";
+}
 struct ScopedPhase {
   Ctx& c;
   int idx;
-  ScopedPhase(Ctx& c_, int phase) : c(c_), idx(c_.timer.begin(phase, c_.stream)) {}
-  ~ScopedPhase() { c.timer.end(idx, c.stream); }
+  ScopedPhase(Ctx& c_, int phase) : c(c_), idx(c_.timer.begin(phase, c_.stream)) { nvtxRangePushA(phase_name(phase)); }
+  ~ScopedPhase() {
+    c.timer.end(idx, c.stream);
+    nvtxRangePop();
+  }
 };
-enum { kPhaseSort = 0, kPhasePush = 1, kPhaseDeposit = 2, kPhaseStray = 3, kPhaseFields = 4 };
 
 // ---- fields.cu
 template <class R> void launch_push_B(const Grid<R>& g, const int lo[3], const int hi[3], Ctx& c);
