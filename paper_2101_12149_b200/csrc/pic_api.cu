@@ -298,6 +298,16 @@ struct Sim : SimBase {
     Species<R> sp;
     sp.q = q;
     sp.m = m;
+    {   // everything this species needs, in one chunk: two buffer sets, cell, perm, tile starts, sort scratch
+      const size_t slack = 512;   // the pool's alignment, per array
+      const size_t nn = (size_t)(n > 0 ? n : 1);
+      size_t need = 2 * (7 * (nn * sizeof(R) + slack) + nn * sizeof(int64_t) + slack) + 2 * (nn * sizeof(int32_t) + slack) +
+                    ((size_t)tile.nt[0] * tile.nt[1] * tile.nt[2] + 1) * sizeof(int32_t) + slack;
+      if (n > scratch.cap)
+        need += 5 * (nn * sizeof(uint32_t) + slack) + ((size_t)sort_hist_len(n) + (size_t)sort_scan_tmp_len(sort_hist_len(n))) * sizeof(uint32_t) +
+                3 * slack;
+      pool.reserve(need);
+    }
     bool ok = alloc_particles(sp.buf[0], n) && alloc_particles(sp.buf[1], n);
     sp.cell = palloc<int32_t>((size_t)(n > 0 ? n : 1));
     sp.perm = palloc<int32_t>((size_t)(n > 0 ? n : 1));
