@@ -156,17 +156,6 @@ __device__ __forceinline__ int cell_of(R x, R inv_dx, int N) {
 __device__ __forceinline__ void red_add(double* p, double v) { atomicAdd(p, v); }
 __device__ __forceinline__ void red_add(float* p, float v) { atomicAdd(p, v); }
 
-// the same, skipped when v == 0, as ONE predicated instruction (no branch around the address arithmetic: the
-// compiler's `if (v != 0) atomicAdd` costs a BSSY / BRA / BSYNC triple per element in the deposit's retire path)
-__device__ __forceinline__ void red_add_nz(double* p, double v) {
-  asm volatile("{\n .reg .pred q;\n setp.neu.f64 q, %1, 0d0000000000000000;\n @q red.global.add.f64 [%0], %1;\n}" ::"l"(p), "d"(v)
-               : "memory");
-}
-__device__ __forceinline__ void red_add_nz(float* p, float v) {
-  asm volatile("{\n .reg .pred q;\n setp.neu.f32 q, %1, 0f00000000;\n @q red.global.add.f32 [%0], %1;\n}" ::"l"(p), "f"(v)
-               : "memory");
-}
-
 // One contribution v to the J element at p (p points into g.J[0..2], which are one allocation). Default: a
 // floating-point reduction at L2, whose result depends on the order of arrival. Deterministic mode: v is
 // split into hi = rint(v 2^e_hi) and lo = rint((v - hi 2^-e_hi) 2^e_lo), both added as 64-bit integers;
@@ -184,15 +173,6 @@ __device__ __forceinline__ void j_add(const Grid<R>& g, R* p, R v) {
     atomicAdd(reinterpret_cast<unsigned long long*>(g.Jfix[1] + off), (unsigned long long)(long long)lo);
   } else {
     red_add(p, v);
-  }
-}
-// j_add for a value that is often exactly zero (untouched accumulator elements)
-template <class R, int DET>
-__device__ __forceinline__ void j_add_nz(const Grid<R>& g, R* p, R v) {
-  if constexpr (DET == 0) {
-    red_add_nz(p, v);
-  } else {
-    if (v != R(0)) j_add<R, DET>(g, p, v);
   }
 }
 

@@ -868,9 +868,9 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
           if (cok[b][c]) {
-            j_add_nz<R, DET>(g, g.J[0] + base + coff[b][c], (R)C.x[b][c]);
-            j_add_nz<R, DET>(g, g.J[1] + base + coff[b][c], (R)C.y[b][c]);
-            j_add_nz<R, DET>(g, g.J[2] + base + coff[b][c], (R)C.z[b][c]);
+            if (C.x[b][c] != 0.0) j_add<R, DET>(g, g.J[0] + base + coff[b][c], (R)C.x[b][c]);
+            if (C.y[b][c] != 0.0) j_add<R, DET>(g, g.J[1] + base + coff[b][c], (R)C.y[b][c]);
+            if (C.z[b][c] != 0.0) j_add<R, DET>(g, g.J[2] + base + coff[b][c], (R)C.z[b][c]);
           }
           C.x[b][c] = 0; C.y[b][c] = 0; C.z[b][c] = 0;
         }
