@@ -251,7 +251,8 @@ def run_reference(args):
     line = {
         "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["ms_per_step"],
-        "ms_per_step_is_for": "%d particles (the timed sample), not the configured %d" % (r["particles"], cfg.n_particles),
+        "ms_per_step_is_for": ("%d particles: the workload at its configured size" % r["particles"]) if r["particles"] == cfg.n_particles
+        else "%d particles (the timed sample), not the configured %d" % (r["particles"], cfg.n_particles),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": cfg.dtype, "data": "synthetic", "config": cd,
         "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
