@@ -73,7 +73,10 @@ enum {
                                  staged in shared memory for gather + push; deposition by
                                  16-lane groups (4 at order 1) that own the (j,k) columns of a
                                  cell's window, sums in registers, one L2 reduction per finished
-                                 window node. AUTO picks this in fp32 when it can. */
+                                 window node. AUTO picks this in fp32 when it can; at order 1 AUTO
+                                 (not an explicit TILE) deposits through the tile's J box in shared
+                                 memory instead: lane = particle, segmented warp reduction per cell
+                                 run, native fp32 shared-memory reductions, one flush per tile. */
   PIC_DEPOSIT_TILE_MMA = 4,   /* as TILE, but the sums of a cell's particles are formed as small
                                  dense contractions on the fp64 tensor pipe (mma.sync m8n8k4.f64),
                                  one warp per cell run (fp64 arithmetic also for PIC_F32 data).

@@ -85,6 +85,7 @@ struct Ctx {
   std::set<const void*> smem_opted;   // kernels whose >48 KB dynamic shared memory opt-in is done for this handle
   // TMA staging of k_push_tile's E/B box (tile_kernels.cu make_push_tensor_map): one 4-D tensor map over the
   // six padded field arrays (x, y, z, component); off when the arrays do not meet TMA's 16-byte stride rule
+  bool auto_deposit = true;   // pic_options.deposit_mode == AUTO: the library may pick a specialised kernel of the mode
   bool tma_push = false;
   alignas(64) CUtensorMap tmap_push;
   int64_t launches = 0;   // kernels launched through this handle

@@ -158,6 +158,7 @@ struct Sim : SimBase {
     dt = dt_;
     sort_interval = o.sort_interval;
     deposit_mode = o.deposit_mode;
+    ctx.auto_deposit = o.deposit_mode == PIC_DEPOSIT_AUTO;
     deterministic = o.deterministic != 0;
     use_graph = o.cuda_graph != 0;
     ctx.stream = (cudaStream_t)o.cuda_stream;

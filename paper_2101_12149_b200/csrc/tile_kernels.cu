@@ -767,6 +767,155 @@ __global__ void __launch_bounds__(NWARP * 32, 2)
   if (cur != INT_MIN) flush_window<R, ORDER, DET>(g, acc, column(cur), curph, grp == 0);
 }
 
+// =================================================================== Esirkepov, fp32 order 1: J of the tile in shared memory
+// north_star's own design ("accumulates J per tile in shared memory with warp-level reductions and then
+// flushes to global memory with atomics"), which fp64 cannot use (64-bit floating-point atomics on shared
+// memory are compare-and-swap loops: measured slower in round 1) but fp32 can: RED.shared.f32 is native. At
+// order 1 a particle touches 4 x 2 x 2 nodes and has 28 non-zero contributions (Jx 3 x 4, Jy 4 x 2, Jz 4 x 2:
+// the last running sum of each axis is zero), few enough for one lane to hold: lane = particle, the lanes of
+// a run of same-cell particles (the sorted order makes them neighbours) are summed with a segmented shuffle
+// reduction, and the head lane of each run adds the 28 sums into the tile's J box in shared memory (11 x 9 x 9
+// nodes); the box goes to global memory once per tile, one reduction per non-zero node. The lane-group kernel
+// k_deposit_tile needs 46 warp instructions per particle for this case (ncu: issue slots 80 % busy: ballots,
+// group shuffles and flushes around 24 FMAs); this one needs ~ 20. Not bit-reproducible from run to run
+// (the order of the shared-memory additions is free), so pic_options.deterministic keeps k_deposit_tile.
+struct SmemCic {
+  static constexpr int BX = 11, BY = 9, BZ = 9;   // nodes tb-1 .. tb+9 along x, tb .. tb+8 along y and z
+  static constexpr int PX = 12;                   // padded x extent
+  static constexpr int VOL = BZ * BY * PX;
+};
+
+__global__ void __launch_bounds__(256, 4)
+    k_deposit_smem_cic(Grid<float> g, Particles<float> p, float* __restrict__ xn, float* __restrict__ yn, float* __restrict__ zn,
+                       const int32_t* __restrict__ tile_start, TileSpec ts, int32_t* __restrict__ stray_list,
+                       unsigned int* __restrict__ stray_count, unsigned long long* deactivated) {
+  using R = float;
+  using B = SmemCic;
+  __shared__ R sJ[3 * B::VOL];
+  const int tile = blockIdx.x;
+  const int s = tile_start[tile], e = tile_start[tile + 1];
+  if (s >= e) return;
+  int tb[3];
+  tile_coords(ts, tile, tb);
+  for (int i = threadIdx.x; i < 3 * B::VOL; i += blockDim.x) sJ[i] = R(0);
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  const R half = R(0.5), third = R(1) / R(3);
+  for (int base = s; base < e; base += blockDim.x) {   // CTA-uniform trip count: whole warps stay together
+    const int t = base + threadIdx.x;
+    const bool valid = t < e;
+    bool elig = false;
+    R x1[3] = {0, 0, 0};
+    R w = 0;
+    int key = -1 - lane;   // particles that do not take part are runs of their own
+    R v[28];
+#pragma unroll
+    for (int i = 0; i < 28; ++i) v[i] = R(0);
+    int node0 = 0;
+    if (valid) {
+      const R x0[3] = {p.x[t], p.y[t], p.z[t]};
+      x1[0] = xn[t]; x1[1] = yn[t]; x1[2] = zn[t];
+      w = p.w[t];
+      R S0x[4], DSx[4], S0y[2], DSy[2], S0z[2], DSz[2];
+      int c[3];
+      bool fit[3];
+      axis_window<R, 1, 4, 1>(mul_rn(x0[0], g.inv_dx[0]), mul_rn(x1[0], g.inv_dx[0]), c[0], S0x, DSx, fit[0]);
+      axis_window<R, 1, 2, 0>(mul_rn(x0[1], g.inv_dx[1]), mul_rn(x1[1], g.inv_dx[1]), c[1], S0y, DSy, fit[1]);
+      axis_window<R, 1, 2, 0>(mul_rn(x0[2], g.inv_dx[2]), mul_rn(x1[2], g.inv_dx[2]), c[2], S0z, DSz, fit[2]);
+      const int rc0 = c[0] - tb[0], rc1 = c[1] - tb[1], rc2 = c[2] - tb[2];
+      elig = fit[0] & fit[1] & fit[2] & (rc0 >= 0) & (rc0 < ts.T[0]) & (rc1 >= 0) & (rc1 < ts.T[1]) & (rc2 >= 0) & (rc2 < ts.T[2]);
+      if (elig) {
+        key = rc0 | (rc1 << 4) | (rc2 << 8);
+        node0 = rc0 + B::PX * (rc1 + B::BY * rc2);   // local node (cell - 1, cell, cell): the window's first node
+        const R fx = -(w * p.jf[0]), fy = -(w * p.jf[1]), fz = -(w * p.jf[2]);
+        // Jx[i][j][k] = fx (DSx[0] + .. + DSx[i]) (S0z[k] (S0y[j] + DSy[j]/2) + DSz[k] (S0y[j]/2 + DSy[j]/3)), i = 0..2
+        R px = 0;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+          px += DSx[i];
+#pragma unroll
+          for (int k = 0; k < 2; ++k)
+#pragma unroll
+            for (int j = 0; j < 2; ++j)
+              v[4 * i + 2 * k + j] = fx * px * (S0z[k] * (S0y[j] + half * DSy[j]) + DSz[k] * (half * S0y[j] + third * DSy[j]));
+        }
+        // Jy[i][0][k] = fy DSy[0] (A[i] S0z[k] + B[i] DSz[k]),  Jz[i][j][0] = fz DSz[0] (A[i] S0y[j] + B[i] DSy[j])
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          const R A = S0x[i] + half * DSx[i], Bc = half * S0x[i] + third * DSx[i];
+#pragma unroll
+          for (int k = 0; k < 2; ++k) v[12 + 2 * i + k] = fy * DSy[0] * (A * S0z[k] + Bc * DSz[k]);
+#pragma unroll
+          for (int j = 0; j < 2; ++j) v[20 + 2 * i + j] = fz * DSz[0] * (A * S0y[j] + Bc * DSy[j]);
+        }
+      }
+    }
+    // runs of equal keys: every lane ends up with the sum over the rest of its run, the head with the whole run
+    const int prev = __shfl_up_sync(0xffffffffu, key, 1);
+    const unsigned heads = __ballot_sync(0xffffffffu, lane == 0 || key != prev);
+    const unsigned after = lane == 31 ? 0u : (heads >> (lane + 1));
+    const int left = after ? __ffs(after) : 32 - lane;   // lanes from this one to the end of its run
+    // (measured on C3: all five steps 0.693 ms, stopping at the longest run of the round 0.644 ms, no
+    // pre-reduction at all — every lane adding into shared memory, 8 lanes per address — 1.98 ms)
+    const int maxleft = __reduce_max_sync(0xffffffffu, left);
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+      if (off >= maxleft) break;
+      const bool take = off < left;
+#pragma unroll
+      for (int i = 0; i < 28; ++i) {
+        const R o = __shfl_down_sync(0xffffffffu, v[i], off);
+        v[i] += take ? o : R(0);
+      }
+    }
+    if (elig && ((heads >> lane) & 1u)) {
+      R* q = sJ + node0;
+#pragma unroll
+      for (int i = 0; i < 3; ++i)
+#pragma unroll
+        for (int k = 0; k < 2; ++k)
+#pragma unroll
+          for (int j = 0; j < 2; ++j) atomicAdd(q + i + B::PX * (j + B::BY * k), v[4 * i + 2 * k + j]);
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+#pragma unroll
+        for (int k = 0; k < 2; ++k) atomicAdd(q + B::VOL + i + B::PX * B::BY * k, v[12 + 2 * i + k]);
+#pragma unroll
+        for (int j = 0; j < 2; ++j) atomicAdd(q + 2 * B::VOL + i + B::PX * j, v[20 + 2 * i + j]);
+      }
+    }
+    // particles deposited here are finished: wrap and store; the others go to the list untouched
+    const bool stray = valid && !elig;
+    const unsigned sm = __ballot_sync(0xffffffffu, stray);
+    if (sm) {
+      unsigned b0 = 0;
+      if (lane == 0) b0 = atomicAdd(stray_count, (unsigned)__popc(sm));
+      b0 = __shfl_sync(0xffffffffu, b0, 0);
+      if (stray) stray_list[b0 + __popc(sm & ((1u << lane) - 1u))] = (int32_t)t;
+    }
+    if (valid && elig) {
+      bool out = false;
+#pragma unroll
+      for (int d = 0; d < 3; ++d) out |= wrap_axis<R>(x1[d], g.L[d], g.periodic[d]);
+      if (out) {
+        if (w != R(0)) atomicAdd(deactivated, 1ull);
+        p.w[t] = R(0);
+      }
+      xn[t] = x1[0]; yn[t] = x1[1]; zn[t] = x1[2];
+    }
+  }
+  __syncthreads();
+  // the tile's box -> J, one reduction per non-zero node; x fastest, so a warp's reductions are contiguous
+  for (int i = threadIdx.x; i < 3 * B::VOL; i += blockDim.x) {
+    const R val = sJ[i];
+    if (val != R(0)) {
+      const int comp = i / B::VOL, r = i % B::VOL;
+      const int lx = r % B::PX, ly = (r / B::PX) % B::BY, lz = r / (B::PX * B::BY);
+      red_add(g.J[comp] + g.idx(tb[0] - 1 + lx, tb[1] + ly, tb[2] + lz), val);
+    }
+  }
+}
+
 // =================================================================== Esirkepov on the fp64 tensor pipe
 // The sums of one cell's particles are small dense contractions over the particles p:
 //   Jx[i][jk] += sum_p PX_p[i] * cx_p[jk]
@@ -1352,9 +1501,21 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, int mo
       kmma<<<n_tiles, mw * 32, mma_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
                                                     a.stray_count, a.deactivated);
     } else {
-      opt_in_smem(c, kvec, vec_smem);
-      kvec<<<n_tiles, kW * 32, vec_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
-                                                    a.stray_count, a.deactivated);
+      bool smem_cic = false;
+      if constexpr (sizeof(R) == 4 && ORDER == 1) {
+        // fp32, order 1, floating-point reductions: the tile's J in shared memory (AUTO's choice; mode TILE given
+        // explicitly keeps the lane-group kernel)
+        if (!det && c.auto_deposit) {
+          smem_cic = true;
+          k_deposit_smem_cic<<<n_tiles, 256, 0, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
+                                                            a.stray_count, a.deactivated);
+        }
+      }
+      if (!smem_cic) {
+        opt_in_smem(c, kvec, vec_smem);
+        kvec<<<n_tiles, kW * 32, vec_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
+                                                      a.stray_count, a.deactivated);
+      }
     }
   }
   c.launches += 2;
