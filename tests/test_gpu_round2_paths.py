@@ -6,7 +6,9 @@
 * the TMA staging of the E/B box against the element-wise cp.async staging: same bits (north_star: "TMA where
   the box is regular"), including tiles smaller than the box (out-of-range parts arrive as zeros) and grids
   whose extents rule TMA out (silent fall-back);
-* the drifted-particle list of k_push_tile overflowing (a tile re-walk instead of an in-line gather).
+* the drifted-particle list of k_push_tile overflowing (a tile re-walk instead of an in-line gather);
+* the fp32 order-1 deposit through the tile's J box in shared memory (k_deposit_smem_cic): small tiles, truncated
+  axes, two species, through a re-sort.
 """
 import numpy as np
 import pytest
@@ -213,3 +215,47 @@ def test_drift_list_overflow_rewalks_the_tile(staging):
     out_of_box = np.any((rel < -0.5) | (rel > 9.5), axis=1)
     counts = np.bincount((tile0[:, 0] // 8) + 2 * (tile0[:, 1] // 8) + 4 * (tile0[:, 2] // 8), weights=out_of_box, minlength=8)
     assert counts.max() > 256, counts
+
+
+@pytest.mark.parametrize("n_cells,tile,periodic", [((16, 16, 16), (8, 8, 8), (1, 1, 1)), ((12, 8, 20), (4, 4, 4), (1, 1, 0)),
+                                                   ((24, 8, 8), (8, 4, 8), (0, 1, 1))])
+def test_fp32_order1_shared_memory_deposit_matches_the_oracle(n_cells, tile, periodic):
+    """k_deposit_smem_cic (AUTO in fp32 at order 1: the tile's J box in shared memory): two species, hot enough
+    that particles cross cell and tile faces, tiles smaller than 8 cells, truncated axes (particles leave and
+    are deactivated, J deposited outside is dropped), several steps through a re-sort; and the same bits of
+    x, u as the lane-group kernel (explicit PIC_DEPOSIT_TILE), which shares nothing but the push with it."""
+    import oracle
+    import paper_2101_12149_b200 as pic
+    cfg = W.scaled(W.CONFIGS["C5"], n_cells, tile=tile, periodic=periodic, dx=(1.0e-6, 0.8e-6, 0.7e-6))
+    cfg.order = 1
+    cfg.dtype = "f32"
+    species, _, _ = W.generate(cfg)
+    E, B = W.random_fields(cfg, np.random.default_rng(11))
+    kw = dict(periodic=periodic, tile=tile, sort_interval=4)
+    o = oracle.Oracle(cfg.n_cells, cfg.dx, cfg.dt, 1, dtype=np.float32, **kw)
+    sims = [pic.Sim(cfg.n_cells, cfg.dx, cfg.dt, 1, dtype=np.float32, deposit_mode=m, **kw) for m in (0, 3)]
+    for spec, arrs in species:
+        a = [arrs[k] for k in ("x", "y", "z", "ux", "uy", "uz", "w")]
+        o.add_species(*a, spec.charge, spec.mass)
+        for g in sims:
+            g.add_species(*a, spec.charge, spec.mass)
+    o.set_fields(E, B)
+    for g in sims:
+        g.set_fields(E, B)
+    o.step(1)
+    for g in sims:
+        g.step(1)
+    compare_state(o, sims[0], TOL32, n_species=2)
+    o.step(5)
+    for g in sims:
+        g.step(5)
+    compare_state(o, sims[0], 20 * TOL32, n_species=2)
+    assert o.diagnostics()["deactivated"] == sims[0].diagnostics()["deactivated"]
+    if 0 in periodic:
+        assert sims[0].diagnostics()["deactivated"] > 0
+    for s in range(2):
+        p0, p1 = sims[0].get_particles(s), sims[1].get_particles(s)
+        assert np.array_equal(p0["id"], p1["id"])
+    J0, J1 = sims[0].get_fields()[2], sims[1].get_fields()[2]
+    scale = max(np.max(np.abs(a)) for a in J1)
+    assert max(np.max(np.abs(a.astype(np.float64) - b)) for a, b in zip(J0, J1)) <= 20 * TOL32 * scale
