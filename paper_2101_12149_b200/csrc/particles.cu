@@ -367,7 +367,7 @@ bool launch_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) 
     launch_tile_kernels<R>(g, a, ORDER, mode, c);
     ScopedPhase ph(c, kPhaseStray);
     auto klist = g.fix_scale[0] != 0.0 ? k_deposit_list_warp<R, ORDER, 1> : k_deposit_list_warp<R, ORDER, 0>;
-    klist<<<c.sm_count * 64, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count, a.deactivated);
+    klist<<<c.sm_count * 8, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count, a.deactivated);
     c.launches += 1;
     return true;
   }

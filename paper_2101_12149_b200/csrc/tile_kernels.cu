@@ -1026,10 +1026,12 @@ __global__ void __launch_bounds__(NWARP * 32, MINB)
     }
   };
 
-  // the warp's contiguous share of the tile, a multiple of 32 particles
+  // the warp's contiguous share of the tile, a multiple of 32 particles; gridDim.y CTAs share a tile when the
+  // grid has too few tiles to fill the machine (C1: 8 tiles)
   const int n = e - s;
-  const int chunk = ((n + NWARP - 1) / NWARP + 31) & ~31;
-  const int wb = s + warp * chunk;
+  const int vwarps = NWARP * (int)gridDim.y;
+  const int chunk = ((n + vwarps - 1) / vwarps + 31) & ~31;
+  const int wb = min(e, s + ((int)blockIdx.y * NWARP + warp) * chunk);
   const int we = min(e, wb + chunk);
 
   for (int rb = wb; rb < we; rb += 32) {
@@ -1498,8 +1500,11 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, int mo
     ScopedPhase ph(c, kPhaseDeposit);
     if (mma) {
       opt_in_smem(c, kmma, mma_smem);
-      kmma<<<n_tiles, mw * 32, mma_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
-                                                    a.stray_count, a.deactivated);
+      // small grids: several CTAs per tile, so that about two waves of CTAs exist
+      int split = 1;
+      while (split < 8 && (int64_t)n_tiles * split * 2 <= (int64_t)c.sm_count * kDepMmaCtas) split *= 2;
+      kmma<<<dim3(n_tiles, split), mw * 32, mma_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, a.stray_list,
+                                                                 a.stray_count, a.deactivated);
     } else {
       bool smem_cic = false;
       if constexpr (sizeof(R) == 4 && ORDER == 1) {
