@@ -255,34 +255,51 @@ def test_C2_full_size_deterministic_deposition_twice():
 
 
 @pytest.mark.skipif(__import__("os").environ.get("PIC_LONG_RUN", "") != "1",
-                    reason="about 6 minutes of host time on 16 cores: set PIC_LONG_RUN=1 (result recorded in DESIGN.md section 8)")
-def test_C2_configured_run_length_against_the_openmp_oracle():
-    """BASELINE.json's headline workload in full — C2 at its configured size for its configured 100 steps —
-    on the CUDA path and on the OpenMP variant of the oracle (pinned to the serial oracle by T12), from the same
-    seeded state: the many-step quantities north_star names (total energy, charge, Gauss residual) are compared
-    every 10 steps, and the particle arrays element by element at the end (ids first: the 25 sorts of the run
-    must have produced the same permutations)."""
-    import oracle
-    cfg = W.CONFIGS["C2"]
+                    reason="minutes to tens of minutes of host time on 16 cores per case: set PIC_LONG_RUN=1 (results recorded in DESIGN.md section 8)")
+@pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
+def test_configured_run_length_against_the_openmp_oracle(name):
+    """BASELINE.json's workloads in full — each config at its configured size for its configured number of steps
+    (C2, C3: 100; C4: 200; C5: 50) — on the CUDA path and on the OpenMP variant of the oracle (pinned to the serial
+    oracle by T12), from the same seeded state: the many-step quantities north_star names (total energy, charge,
+    Gauss residual) are compared at ten checkpoints, and the particle arrays element by element at the end (ids
+    first: every sort of the run must have produced the same permutation)."""
+    cfg = W.CONFIGS[name]
     o, g, _ = make_pair(cfg)
+    nsp = len(cfg.species)
+    per = cfg.steps // 10
     hist = []
     for k in range(10):
-        g.step(10)
-        o.step_omp(10)
+        g.step(per)
+        o.step_omp(per)
         dg, do = g.diagnostics(), o.diagnostics()
         eg = dg["field_E"] + dg["field_B"] + dg["kinetic"]
         eo = do["field_E"] + do["field_B"] + do["kinetic"]
-        hist.append((10 * (k + 1), eg, eo, dg["kinetic"], do["kinetic"]))
+        hist.append((per * (k + 1), eg, eo, dg["kinetic"], do["kinetic"], dg["deactivated"], do["deactivated"]))
+        print("%4d %.12e %.12e %.12e %.12e %d %d" % hist[-1], flush=True)
         assert abs(eg - eo) <= 1e-3 * abs(eo), hist
-        assert abs(dg["field_E"] - do["field_E"]) <= 1e-3 * max(abs(do["field_E"]), 1e-30), hist
-        assert dg["charge"] == pytest.approx(do["charge"], rel=1e-12)
-        assert abs(dg["gauss_max"] - do["gauss_max"]) <= 1e-9 * max(do["rho_max"], do["gauss_max"])
-    print("steps, total energy (CUDA), total energy (oracle), kinetic (CUDA), kinetic (oracle):")
-    for row in hist:
-        print("%4d %.12e %.12e %.12e %.12e" % row)
-    pg, po = g.get_particles(0), o.get_particles(0)
-    assert np.array_equal(pg["id"], po["id"])
-    ex = family_err([pg[k] for k in "xyz"], [po[k] for k in "xyz"])
-    eu = family_err([pg[k] for k in ("ux", "uy", "uz")], [po[k] for k in ("ux", "uy", "uz")])
-    print("after 100 steps: max position error %.2e of L, max momentum error %.2e of max|u|" % (ex, eu))
-    assert ex <= 1e-9 and eu <= 1e-9
+        assert abs(dg["kinetic"] - do["kinetic"]) <= 1e-3 * abs(do["kinetic"]) + 1e-30, hist
+        assert abs(dg["charge"] - do["charge"]) <= (1e-12 if cfg.dtype == "f64" else 1e-6) * max(abs(do["charge"]), W.Q_E * 1e25 * 1e-18 * 1e3)
+        assert abs(dg["gauss_max"] - do["gauss_max"]) <= (1e-9 if cfg.dtype == "f64" else 1e-3) * max(do["rho_max"], do["gauss_max"])
+        assert dg["deactivated"] == do["deactivated"]
+    for s in range(nsp):
+        pg, po = g.get_particles(s), o.get_particles(s)
+        moved = int(np.sum(pg["id"] != po["id"]))
+        if cfg.dtype == "f64":
+            assert moved == 0           # every sort of the run produced the same permutation
+        # fp32: J differs in the last bits (summation order), so after many steps a particle next to a cell face can
+        # fall on the other side of it and the sorted orders differ in a few slots: compare particle by particle
+        ig, io = np.argsort(pg["id"]), np.argsort(po["id"])
+        ex = 0.0
+        for d, k in enumerate("xyz"):
+            L = cfg.n_cells[d] * cfg.dx[d]
+            dd = np.abs(pg[k][ig].astype(np.float64) - po[k][io])
+            if cfg.periodic[d]:
+                dd = np.minimum(dd, L - dd)          # a particle next to the seam may sit on either side of it
+            ex = max(ex, float(dd.max()) / L)
+            del dd
+        eu = family_err([pg[k][ig] for k in ("ux", "uy", "uz")], [po[k][io] for k in ("ux", "uy", "uz")])
+        print("%s species %d after %d steps: %d of %d slots hold another particle; max position error %.2e of L, "
+              "max momentum error %.2e of max|u|" % (name, s, cfg.steps, moved, len(ig), ex, eu), flush=True)
+        del ig, io
+        assert ex <= (1e-9 if cfg.dtype == "f64" else 1e-3) and eu <= (1e-9 if cfg.dtype == "f64" else 1e-2)
+        del pg, po
