@@ -1,19 +1,24 @@
 // Tile-centric particle kernels: one CTA per particle tile (<= 8x8x8 cells,
 // the bins of the sort). After a sort the particles of a tile are one contiguous
-// range [tile_start[t], tile_start[t+1]) in cell order, which gives both kernels their locality:
-//   k_push_tile     stages the tile's E/B stencil box in shared memory once, then gathers and
-//                   pushes one particle per thread from it (gather + push fused, no
-//                   per-particle E/B in memory);
-//   k_deposit_tile  Esirkepov deposition (ref [8]) by groups of 16 lanes (4 at
-//                   order 1): the lanes of a group own the (j,k) columns of a cell's window, x runs
-//                   along registers (slot = node mod NX, so nothing moves when the window advances),
-//                   the groups of a warp take the particles of one cell together, and every
-//                   finished window node is one reduction at L2;
-//   k_deposit_mma   the same sums as 8 x 16 x K contractions on the fp64 tensor pipe, one warp per
-//                   run of same-cell particles (the fp64 default).
-// Particles that do not fit a kernel's windows (they crossed a cell face in y or z this step, or
-// drifted too far from the tile since the last sort) go to a list and are deposited one thread each
-// (particles.cu); correctness never depends on the order or the tile.
+// range [tile_start[t], tile_start[t+1]) in cell order, which gives the kernels their locality:
+//   k_push_tile         stages the tile's E/B stencil box in shared memory once — one TMA bulk tensor copy
+//                       (cp.async.bulk.tensor + mbarrier) or element-wise cp.async — then gathers and
+//                       pushes one particle per thread from it (gather + push fused, no
+//                       per-particle E/B in memory);
+//   k_deposit_mma       Esirkepov deposition (ref [8]) as 8 x 16 x K contractions on the
+//                       fp64 tensor pipe, one warp per round of 32 particles grouped by cell triple
+//                       (the fp64 default);
+//   k_deposit_tile      the same sums by groups of 16 lanes (4 at order 1): the lanes of a group own the
+//                       (j,k) columns of a cell's window, x runs along registers (slot = node mod NX, so
+//                       nothing moves when the window advances), every finished window node is one
+//                       reduction at L2 (the fp32 default at orders 2 and 3);
+//   k_deposit_smem_cic  fp32 order 1: lane = particle, segmented warp reduction per cell run, the tile's J
+//                       box in shared memory, one flush per tile (the fp32 default at order 1);
+//   k_fused_mma         gather + push + tensor-pipe deposit in one kernel (measured slower, on request).
+// A particle that crosses one cell face in y or z stays in the deposit kernels (its one extra node is
+// added by the warp, extra_node_deposit); particles that cross in y and z at once, or drifted too far
+// from the tile since the last sort, go to a list and are deposited one warp each (particles.cu);
+// correctness never depends on the order or the tile.
 #include <algorithm>
 #include <climits>
 #include <type_traits>
