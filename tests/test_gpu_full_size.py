@@ -278,7 +278,14 @@ def test_configured_run_length_against_the_openmp_oracle(name):
         print("%4d %.12e %.12e %.12e %.12e %d %d" % hist[-1], flush=True)
         assert abs(eg - eo) <= 1e-3 * abs(eo), hist
         assert abs(dg["kinetic"] - do["kinetic"]) <= 1e-3 * abs(do["kinetic"]) + 1e-30, hist
-        assert abs(dg["charge"] - do["charge"]) <= (1e-12 if cfg.dtype == "f64" else 1e-6) * max(abs(do["charge"]), W.Q_E * 1e25 * 1e-18 * 1e3)
+        # total charge = sum of q w over all particles: with unequal weights (C4's ramp) the oracle's sequential sum
+        # and the GPU's tree differ by summation-order rounding, up to N eps; what must hold exactly is that
+        # neither side's charge changes while no particle leaves
+        assert abs(dg["charge"] - do["charge"]) <= (1e-8 if cfg.dtype == "f64" else 1e-5) * max(abs(do["charge"]), W.Q_E * 1e25 * 1e-18 * 1e3)
+        if k == 0:
+            q0 = (dg["charge"], do["charge"])
+        elif dg["deactivated"] == 0:
+            assert dg["charge"] == pytest.approx(q0[0], rel=1e-13) and do["charge"] == pytest.approx(q0[1], rel=1e-13)
         assert abs(dg["gauss_max"] - do["gauss_max"]) <= (1e-9 if cfg.dtype == "f64" else 1e-3) * max(do["rho_max"], do["gauss_max"])
         assert dg["deactivated"] == do["deactivated"]
     for s in range(nsp):
