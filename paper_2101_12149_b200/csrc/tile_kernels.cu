@@ -777,12 +777,12 @@ __global__ void __launch_bounds__(NWARP * 32, 2)
 // flushes to global memory with atomics"), which fp64 cannot use (64-bit floating-point atomics on shared
 // memory are compare-and-swap loops: measured slower in round 1) but fp32 can: RED.shared.f32 is native. At
 // order 1 a particle touches 4 x 2 x 2 nodes and has 28 non-zero contributions (Jx 3 x 4, Jy 4 x 2, Jz 4 x 2:
-// the last running sum of each axis is zero), few enough for one lane to hold: lane = particle, the lanes of
-// a run of same-cell particles (the sorted order makes them neighbours) are summed with a segmented shuffle
-// reduction, and the head lane of each run adds the 28 sums into the tile's J box in shared memory (11 x 9 x 9
-// nodes); the box goes to global memory once per tile, one reduction per non-zero node. The lane-group kernel
+// the last running sum of each axis is zero), few enough for one lane to hold: lane = particle; the 28 x 32
+// values of a round are transposed through shared memory, lane l sums value l over every run of same-cell
+// particles (the sorted order makes them neighbours) and adds the sums into the tile's J box in shared memory
+// (11 x 9 x 9 nodes); the box goes to global memory once per tile, one reduction per non-zero node. The lane-group kernel
 // k_deposit_tile needs 46 warp instructions per particle for this case (ncu: issue slots 80 % busy: ballots,
-// group shuffles and flushes around 24 FMAs); this one needs ~ 20. Not bit-reproducible from run to run
+// group shuffles and flushes around 24 FMAs); this one needs about half. Not bit-reproducible from run to run
 // (the order of the shared-memory additions is free), so pic_options.deterministic keeps k_deposit_tile.
 struct SmemCic {
   static constexpr int BX = 11, BY = 9, BZ = 9;   // nodes tb-1 .. tb+9 along x, tb .. tb+8 along y and z
@@ -797,6 +797,8 @@ __global__ void __launch_bounds__(256, 4)
   using R = float;
   using B = SmemCic;
   __shared__ R sJ[3 * B::VOL];
+  __shared__ R s_val[8 * 28 * 33];   // per warp: 28 values x 32 particles, row stride 33 (conflict-free both ways)
+  __shared__ int s_node[8 * 32];
   const int tile = blockIdx.x;
   const int s = tile_start[tile], e = tile_start[tile + 1];
   if (s >= e) return;
@@ -806,6 +808,11 @@ __global__ void __launch_bounds__(256, 4)
   __syncthreads();
   const int lane = threadIdx.x & 31;
   const R half = R(0.5), third = R(1) / R(3);
+  // the box element (relative to the window's first node) that value `lane` of the 28 belongs to
+  int my_off = 0;
+  if (lane < 12) my_off = lane / 4 + B::PX * ((lane & 1) + B::BY * ((lane >> 1) & 1));
+  else if (lane < 20) my_off = B::VOL + (lane - 12) / 2 + B::PX * B::BY * ((lane - 12) & 1);
+  else if (lane < 28) my_off = 2 * B::VOL + (lane - 20) / 2 + B::PX * ((lane - 20) & 1);
   for (int base = s; base < e; base += blockDim.x) {   // CTA-uniform trip count: whole warps stay together
     const int t = base + threadIdx.x;
     const bool valid = t < e;
@@ -855,39 +862,32 @@ __global__ void __launch_bounds__(256, 4)
         }
       }
     }
-    // runs of equal keys: every lane ends up with the sum over the rest of its run, the head with the whole run
+    // runs of equal keys (the sorted order makes same-cell particles neighbours): their 28 sums go to the J box
     const int prev = __shfl_up_sync(0xffffffffu, key, 1);
     const unsigned heads = __ballot_sync(0xffffffffu, lane == 0 || key != prev);
-    const unsigned after = lane == 31 ? 0u : (heads >> (lane + 1));
-    const int left = after ? __ffs(after) : 32 - lane;   // lanes from this one to the end of its run
-    // (measured on C3: all five steps 0.693 ms, stopping at the longest run of the round 0.644 ms, no
-    // pre-reduction at all — every lane adding into shared memory, 8 lanes per address — 1.98 ms)
-    const int maxleft = __reduce_max_sync(0xffffffffu, left);
+    // transposed through shared memory: lane p stores its 28 values as a column, lane l then walks ROW l over the
+    // 32 particles and adds the sum of every run into the box (the run boundaries are warp-uniform): 28 stores +
+    // 32 loads per lane. Measured on C3: 0.469 ms; the same sums by a segmented shuffle reduction (28 values x up
+    // to 5 steps, head lanes adding) 0.645 ms; every lane adding its own values (8 lanes per address) 1.98 ms
+    {
+      R* sv = s_val + (threadIdx.x >> 5) * (28 * 33);
+      int* sn = s_node + (threadIdx.x >> 5) * 32;
 #pragma unroll
-    for (int off = 1; off < 32; off <<= 1) {
-      if (off >= maxleft) break;
-      const bool take = off < left;
+      for (int i = 0; i < 28; ++i) sv[i * 33 + lane] = v[i];
+      sn[lane] = elig ? node0 : -1;
+      __syncwarp();
+      const R* row = sv + (lane < 28 ? lane : 0) * 33;
+      R acc = 0;
 #pragma unroll
-      for (int i = 0; i < 28; ++i) {
-        const R o = __shfl_down_sync(0xffffffffu, v[i], off);
-        v[i] += take ? o : R(0);
+      for (int q = 0; q < 32; ++q) {
+        acc += row[q];
+        if (q == 31 || ((heads >> (q + 1)) & 1u)) {   // warp-uniform
+          const int n0 = sn[q];
+          if (n0 >= 0 && lane < 28) atomicAdd(sJ + n0 + my_off, acc);
+          acc = 0;
+        }
       }
-    }
-    if (elig && ((heads >> lane) & 1u)) {
-      R* q = sJ + node0;
-#pragma unroll
-      for (int i = 0; i < 3; ++i)
-#pragma unroll
-        for (int k = 0; k < 2; ++k)
-#pragma unroll
-          for (int j = 0; j < 2; ++j) atomicAdd(q + i + B::PX * (j + B::BY * k), v[4 * i + 2 * k + j]);
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-#pragma unroll
-        for (int k = 0; k < 2; ++k) atomicAdd(q + B::VOL + i + B::PX * B::BY * k, v[12 + 2 * i + k]);
-#pragma unroll
-        for (int j = 0; j < 2; ++j) atomicAdd(q + 2 * B::VOL + i + B::PX * j, v[20 + 2 * i + j]);
-      }
+      __syncwarp();
     }
     // particles deposited here are finished: wrap and store; the others go to the list untouched
     const bool stray = valid && !elig;
