@@ -170,7 +170,10 @@ __device__ __forceinline__ void push_store(const Grid<R>& g, const Particles<R>&
 // are one allocation, described as a 4-D tensor), signalled on an mbarrier; meanwhile every thread already
 // loads its first particle. Otherwise 6 * EXT^3 element-wise cp.async copies.
 template <class R, int ORDER, int PUSHER, int GATHER, bool TMA>
-__global__ void __launch_bounds__(kPushTileThreads, 2) k_push_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn,
+// Register budget: two CTAs per SM (128 registers) where the box needs the shared memory anyway; fp32 at order
+// 1 (25 KB box) is latency-bound instead and runs best with four (64 registers; C3 push by CTAs per SM:
+// 2: 0.395 ms, 3: 0.333, 4: 0.316, 5: 0.318, 6: 0.334)
+__global__ void __launch_bounds__(kPushTileThreads, (sizeof(R) == 4 && ORDER == 1) ? 4 : 2) k_push_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn,
                                                                    R* __restrict__ yn, R* __restrict__ zn,
                                                                    const int32_t* __restrict__ tile_start, TileSpec ts,
                                                                    const __grid_constant__ CUtensorMap tmap) {
