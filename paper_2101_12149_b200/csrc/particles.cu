@@ -10,6 +10,8 @@
 // ref [8] Esirkepov PAPER.md:301.
 #include <climits>
 
+#include <algorithm>
+
 #include "internal.h"
 #include "particle_math.cuh"
 
@@ -367,7 +369,12 @@ bool launch_order(const Grid<R>& g, const ParticleStep<R>& a, int mode, Ctx& c) 
     launch_tile_kernels<R>(g, a, ORDER, mode, c);
     ScopedPhase ph(c, kPhaseStray);
     auto klist = g.fix_scale[0] != 0.0 ? k_deposit_list_warp<R, ORDER, 1> : k_deposit_list_warp<R, ORDER, 0>;
-    klist<<<c.sm_count * 8, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count, a.deactivated);
+    // one warp per listed particle, grid-stride; the list length is only known on the device, so the grid is sized
+    // from the species: enough warps in flight for a large one (each listed particle is a chain of dependent
+    // loads), few CTAs for a small one (an empty CTA still costs its launch)
+    const int64_t want = p.n / 1024;
+    const int blocks = (int)std::min<int64_t>((int64_t)c.sm_count * 64, std::max<int64_t>(c.sm_count, want));
+    klist<<<blocks, 128, 0, c.stream>>>(g, p, xn, yn, zn, a.stray_list, a.stray_count, a.deactivated);
     c.launches += 1;
     return true;
   }
