@@ -122,7 +122,10 @@ template <class R> void launch_unpack(const Grid<R>& g, const R* padded_src, R* 
 
 // ---- particles.cu
 enum { kDepositGlobal = 1, kDepositCoop = 2, kDepositTile = 3, kDepositTileMma = 4, kDepositFused = 5 };
-constexpr int kPushTileThreads = 256;   // k_push_tile: threads per CTA (one CTA per tile)
+// k_push_tile: threads per CTA (one CTA per tile). fp64: 12 warps per SM (two CTAs) already saturate the shared-memory
+// path and 192 threads measured best (C2 push: 128: 1.672 ms, 160: 1.668, 192: 1.612, 224: 1.696, 256: 1.634, 320: 1.875);
+// fp32 is latency-bound and wants the warps (C3: 0.316 ms at 256 against 0.331 at 192)
+template <class R> constexpr int kPushTileThreads = sizeof(R) == 8 ? 192 : 256;
 constexpr int kDepMmaWarps = 4;         // k_deposit_mma: warps per CTA (one CTA per tile) ...
 constexpr int kDepMmaCtas = 5;          // ... and CTAs per SM the register budget is set for (20 warps per SM)
 constexpr int kFusedWarps = 12;         // k_fused_mma: warps per CTA (one CTA per tile, one per SM: box + 12 record buffers = 216 KB)

@@ -173,7 +173,7 @@ template <class R, int ORDER, int PUSHER, int GATHER, bool TMA>
 // Register budget: two CTAs per SM (128 registers) where the box needs the shared memory anyway; fp32 at order
 // 1 (25 KB box) is latency-bound instead and runs best with four (64 registers; C3 push by CTAs per SM:
 // 2: 0.395 ms, 3: 0.333, 4: 0.316, 5: 0.318, 6: 0.334)
-__global__ void __launch_bounds__(kPushTileThreads, (sizeof(R) == 4 && ORDER == 1) ? 4 : 2) k_push_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn,
+__global__ void __launch_bounds__(kPushTileThreads<R>, (sizeof(R) == 4 && ORDER == 1) ? 4 : 2) k_push_tile(Grid<R> g, Particles<R> p, R* __restrict__ xn,
                                                                    R* __restrict__ yn, R* __restrict__ zn,
                                                                    const int32_t* __restrict__ tile_start, TileSpec ts,
                                                                    const __grid_constant__ CUtensorMap tmap) {
@@ -1502,7 +1502,7 @@ static void launch_tile_order(const Grid<R>& g, const ParticleStep<R>& a, int mo
     };
     auto kpush = tma ? pick(std::true_type{}) : pick(std::false_type{});
     opt_in_smem(c, kpush, push_smem);
-    kpush<<<n_tiles, kPushTileThreads, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, c.tmap_push);
+    kpush<<<n_tiles, kPushTileThreads<R>, push_smem, c.stream>>>(g, p, xn, yn, zn, a.tile_start, a.tiles, c.tmap_push);
   }
   {
     ScopedPhase ph(c, kPhaseDeposit);
