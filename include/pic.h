@@ -273,6 +273,25 @@ PIC_API int pic_probe_peaks(void* cuda_stream, double seconds_per_probe, double*
  * alpha[3], beta[9], gamma[3]. Errors: INVALID_ARG. */
 PIC_API int pic_ckc_coefficients(const double dx[3], double alpha[3], double beta[9], double gamma[3]);
 
+/* The sort of step 1 for callers that may NOT allocate: code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc. Computes, for n particles at
+ * positions x, y, z, exactly what pic_sort_now + pic_get_sort_state give — perm[k] = the input slot of the
+ * particle that the stable sort by tile-major cell key puts at slot k, cell[k] = its cell index
+ * cx + Nx*(cy + Ny*cz) — with the same kernels, and makes no cudaMalloc / cudaFree / pool call: the scratch of
+ * the radix passes is ONE file-scope device array of fixed size inside the library (about 8.3 MB, held by every
+ * GPU that loads the library until the process exits). Hence the limit n <= PIC_NOALLOC_MAX_PARTICLES
+ * (PIC_ERR_CAPACITY beyond it, with a message in pic_last_error(NULL)).
+ * x, y, z, cell, perm are DEVICE pointers (elements of prec; int32 outputs of n entries); n_cells, dx, tile are
+ * host arrays with the meaning they have in pic_create / pic_options (a tile larger than the grid is clipped).
+ * No particle data is moved; no handle is involved. Asynchronous on cuda_stream (NULL = the legacy default
+ * stream); runs on the current device. All calls on one device share the scratch array: two calls that overlap
+ * on the GPU (different streams without a dependency) race — order them. Nothing is kept between calls.
+ * Errors: INVALID_ARG, CAPACITY, CUDA. */
+#define PIC_NOALLOC_MAX_PARTICLES 524288
+PIC_API int pic_sort_permutation_noalloc(const int32_t n_cells[3], const double dx[3], const int32_t tile[3],
+                                         int32_t sort_key_mode, pic_precision prec, const void* x, const void* y,
+                                         const void* z, int64_t n, int32_t* cell, int32_t* perm, void* cuda_stream);
+
 /* Free everything the handle owns (synchronises). NULL is a no-op. */
 PIC_API void pic_destroy(pic_sim* sim);
 

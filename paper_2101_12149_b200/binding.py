@@ -33,8 +33,9 @@ SYMBOLS = (
     "pic_default_options", "pic_create", "pic_add_species", "pic_set_fields", "pic_step", "pic_synchronize",
     "pic_get_fields", "pic_get_particles", "pic_get_sort_state", "pic_sort_now", "pic_get_diagnostics",
     "pic_get_rho", "pic_enable_phase_timing", "pic_get_phase_times", "pic_num_particles", "pic_num_species",
-    "pic_last_error", "pic_ckc_coefficients", "pic_probe_peaks", "pic_destroy",
+    "pic_last_error", "pic_ckc_coefficients", "pic_probe_peaks", "pic_destroy", "pic_sort_permutation_noalloc",
 )
+PIC_NOALLOC_MAX_PARTICLES = 524288
 
 
 class PicError(RuntimeError):
@@ -89,6 +90,7 @@ def lib():
         L.pic_probe_peaks.argtypes = [vp, C.c_double, dp]
         L.pic_destroy.argtypes = [vp]
         L.pic_destroy.restype = None
+        L.pic_sort_permutation_noalloc.argtypes = [i32p, dp, i32p, C.c_int32, C.c_int, vp, vp, vp, C.c_int64, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -232,6 +234,30 @@ def pic_ckc_coefficients(dx):
     if rc != 0:
         raise PicError(rc, "dx must be positive and finite")
     return np.array(al[:]), np.array(be[:]).reshape(3, 3), np.array(ga[:])
+
+
+def pic_sort_permutation_noalloc(n_cells, dx, tile, x, y, z, cell, perm, sort_key_mode=0, stream=None):
+    """Allocation-free sort (include/pic.h): x, y, z are device arrays of one dtype (float64 / float32), cell and perm
+    int32 device arrays of the same length; asynchronous on `stream`."""
+    n = _n_elems(x)
+    dt = np.float64 if _elem_size(x) == 8 else np.float32
+    rc = lib().pic_sort_permutation_noalloc(
+        (C.c_int32 * 3)(*[int(v) for v in n_cells]), (C.c_double * 3)(*[float(v) for v in dx]),
+        (C.c_int32 * 3)(*[int(v) for v in tile]), int(sort_key_mode), PIC_F64 if dt == np.float64 else PIC_F32,
+        _dev_ptr(x), _dev_ptr(y), _dev_ptr(z), n, _dev_ptr(cell), _dev_ptr(perm), stream)
+    _check(None, rc)
+
+
+def _dev_ptr(t):
+    return int(t.data_ptr()) if hasattr(t, "data_ptr") else int(t)
+
+
+def _n_elems(t):
+    return int(t.numel())
+
+
+def _elem_size(t):
+    return int(t.element_size())
 
 
 PROBE_NAMES = ("fp64_fma_tflops", "fp64_mma_tflops", "smem_tbs", "fp32_fma_tflops", "sm_count", "sm_clock_mhz")

@@ -4,6 +4,7 @@
 #include <cuda.h>   // CUtensorMap (types only: the encoder is fetched with cudaGetDriverEntryPoint, nothing links libcuda)
 
 #include <set>
+#include <string>
 #include <vector>
 
 #include "common.cuh"
@@ -110,6 +111,9 @@ struct ScopedPhase {
     nvtxRangePop();
   }
 };
+
+// ---- pic_api.cu: the text pic_last_error(NULL) returns, for handle-less entry points in other files
+void set_handleless_error(const std::string& msg);
 
 // ---- fields.cu
 template <class R> void launch_push_B(const Grid<R>& g, const int lo[3], const int hi[3], Ctx& c);

@@ -708,6 +708,10 @@ struct Sim : SimBase {
 };
 
 }  // namespace
+
+// for entry points outside this file that have no handle: the text pic_last_error(NULL) returns (this thread)
+void set_handleless_error(const std::string& msg) { g_create_error = msg; }
+
 }  // namespace pic
 
 struct pic_sim {

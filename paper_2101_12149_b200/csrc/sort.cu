@@ -4,7 +4,12 @@
 // pass, least significant first); every pass is itself a stable counting sort: per-block digit
 // histogram -> exclusive prefix sum -> order-preserving scatter. Stability makes the final
 // permutation unique, so it can be compared bit for bit.
+#include <cmath>
+#include <mutex>
+#include <string>
+
 #include "internal.h"
+#include "pic.h"
 
 namespace pic {
 
@@ -267,4 +272,140 @@ template void sort_species<double>(const Grid<double>&, const TileSpec&, const P
 template void sort_species<float>(const Grid<float>&, const TileSpec&, const Particles<float>&,
                                   const Particles<float>&, int32_t*, int32_t*, int32_t*, SortScratch&, Ctx&);
 
+// =================================================================== the sort without any allocation
+// pic_sort_permutation_noalloc (include/pic.h): the same stable sort by tile-major cell key (same key kernel,
+// same radix passes, same scan) for callers that may not allocate — code under CUDA graph capture, serving
+// loops, harnesses that forbid cudaMalloc. The scratch the passes need (two key and two value buffers, the
+// per-block digit histogram, the block sums of the scan) lives in ONE file-scope device array of fixed size,
+// so the call makes no cudaMalloc / cudaFree and touches no pool. Every GPU that loads the library holds the
+// array (kNoAllocBytes, about 8.3 MB) until the process exits; every call on a device shares it, so two calls
+// that overlap on the GPU (different streams, no dependency) race. Nothing in it has to start at zero — every
+// region is written before it is read within a call (keys/values by k_make_keys, every histogram entry by
+// k_radix_hist, the block sums by k_scan_block) — the histogram is cleared all the same, for a defined state.
+namespace {
+
+constexpr int64_t kNoAllocMaxN = PIC_NOALLOC_MAX_PARTICLES;                               // 524 288
+constexpr int64_t kNoAllocBlocks = (kNoAllocMaxN + kSortChunk - 1) / kSortChunk;           // 128 radix blocks
+constexpr int64_t kNoAllocHist = 256 * kNoAllocBlocks;                                     // digit-major histogram
+constexpr int64_t kNoAllocScan = 64;                                                       // >= sort_scan_tmp_len(kNoAllocHist)
+constexpr int64_t kNoAllocWords = 4 * kNoAllocMaxN + kNoAllocHist + kNoAllocScan;
+constexpr int64_t kNoAllocBytes = kNoAllocWords * (int64_t)sizeof(uint32_t);
+
+// In host code this name is a host-side stand-in for the symbol, NOT a device address: the address the
+// kernels get comes from cudaGetSymbolAddress (noalloc_scratch below), once per device.
+static __device__ __align__(256) uint32_t g_noalloc_scratch[kNoAllocWords];
+
+constexpr int kMaxDevices = 64;
+uint32_t* g_noalloc_ptr[kMaxDevices] = {};   // per device ordinal; written once, under the mutex
+std::mutex g_noalloc_mutex;
+
+// device address of the scratch array on the CURRENT device (looked up once per device, with it current)
+cudaError_t noalloc_scratch(uint32_t** out) {
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+  if (!g_noalloc_ptr[dev]) {
+    uint32_t* ptr = nullptr;
+    e = cudaGetSymbolAddress((void**)&ptr, g_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    g_noalloc_ptr[dev] = ptr;
+  }
+  *out = g_noalloc_ptr[dev];
+  return cudaSuccess;
+}
+
+// what k_permute records, without moving any particle data: perm[k] = source slot, cell[k] = its cell
+template <class R>
+__global__ void __launch_bounds__(256) k_perm_cell(Grid<R> g, const R* __restrict__ x, const R* __restrict__ y,
+                                                   const R* __restrict__ z, int64_t n, const uint32_t* __restrict__ order,
+                                                   int32_t* __restrict__ cell, int32_t* __restrict__ perm) {
+  int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= n) return;
+  uint32_t s = order[k];
+  perm[k] = (int32_t)s;
+  int cx = cell_of<R>(x[s], g.inv_dx[0], g.N[0]);
+  int cy = cell_of<R>(y[s], g.inv_dx[1], g.N[1]);
+  int cz = cell_of<R>(z[s], g.inv_dx[2], g.N[2]);
+  cell[k] = cx + g.N[0] * (cy + g.N[1] * cz);
+}
+
+template <class R>
+cudaError_t sort_permutation_noalloc(const int32_t* n_cells, const double* dx, const TileSpec& t, const R* x, const R* y,
+                                     const R* z, int64_t n, int32_t* cell, int32_t* perm, cudaStream_t stream) {
+  uint32_t* base = nullptr;
+  cudaError_t e = noalloc_scratch(&base);
+  if (e != cudaSuccess) return e;
+  uint32_t* keys[2] = {base, base + kNoAllocMaxN};
+  uint32_t* vals[2] = {base + 2 * kNoAllocMaxN, base + 3 * kNoAllocMaxN};
+  uint32_t* hist = base + 4 * kNoAllocMaxN;
+  uint32_t* scan_tmp = hist + kNoAllocHist;
+  Grid<R> g{};
+  for (int d = 0; d < 3; ++d) {
+    g.N[d] = n_cells[d];
+    g.inv_dx[d] = (R)(1.0 / dx[d]);   // as pic_create rounds it
+  }
+  Ctx c;
+  c.stream = stream;
+  e = cudaMemsetAsync(hist, 0, (size_t)kNoAllocHist * sizeof(uint32_t), stream);
+  if (e != cudaSuccess) return e;
+  const int nblocks = (int)((n + kSortChunk - 1) / kSortChunk);
+  k_make_keys<R><<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(g, t, x, y, z, n, keys[0], vals[0]);
+  const int bits = key_bits(t);
+  int in = 0;
+  for (int shift = 0; shift < bits; shift += 8) {
+    k_radix_hist<<<nblocks, kSortThreads, 0, stream>>>(keys[in], n, shift, hist, nblocks);
+    scan_exclusive(hist, 256 * (int64_t)nblocks, scan_tmp, c);
+    k_radix_scatter<<<nblocks, kSortThreads, 0, stream>>>(keys[in], vals[in], keys[in ^ 1], vals[in ^ 1], n, shift, hist,
+                                                          nblocks);
+    in ^= 1;
+  }
+  k_perm_cell<R><<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(g, x, y, z, n, vals[in], cell, perm);
+  return cudaGetLastError();
+}
+
+}  // namespace
+
 }  // namespace pic
+
+extern "C" PIC_API int pic_sort_permutation_noalloc(const int32_t n_cells[3], const double dx[3], const int32_t tile[3],
+                                                    int32_t sort_key_mode, pic_precision prec, const void* x, const void* y,
+                                                    const void* z, int64_t n, int32_t* cell, int32_t* perm, void* cuda_stream) {
+  using namespace pic;
+  auto bad = [&](int code, const std::string& msg) { set_handleless_error(msg); return code; };
+  if (!n_cells || !dx || !tile) return bad(PIC_ERR_INVALID_ARG, "null grid description");
+  if (prec != PIC_F64 && prec != PIC_F32) return bad(PIC_ERR_INVALID_ARG, "unknown precision");
+  if (sort_key_mode < 0 || sort_key_mode > 1) return bad(PIC_ERR_INVALID_ARG, "sort_key_mode must be 0 or 1");
+  if (n < 0) return bad(PIC_ERR_INVALID_ARG, "negative particle count");
+  if (n > kNoAllocMaxN)
+    return bad(PIC_ERR_CAPACITY, "pic_sort_permutation_noalloc: n = " + std::to_string(n) + " exceeds PIC_NOALLOC_MAX_PARTICLES = " +
+                                     std::to_string(kNoAllocMaxN) + " (the fixed scratch array); use pic_sort_now on a handle");
+  TileSpec t{};
+  uint64_t nnodes = 1;
+  for (int d = 0; d < 3; ++d) {
+    if (n_cells[d] < 1) return bad(PIC_ERR_INVALID_ARG, "n_cells must be at least 1 on every axis");
+    if (!(dx[d] > 0) || !std::isfinite(dx[d])) return bad(PIC_ERR_INVALID_ARG, "dx must be positive and finite");
+    if (tile[d] < 1) return bad(PIC_ERR_INVALID_ARG, "tile must be at least 1");
+    const int T = tile[d] < n_cells[d] ? tile[d] : n_cells[d];
+    if (n_cells[d] % T != 0) return bad(PIC_ERR_INVALID_ARG, "tile must divide n_cells");
+    t.T[d] = T;
+    t.nt[d] = n_cells[d] / T;
+    nnodes *= (uint64_t)n_cells[d];
+  }
+  if (nnodes >= (1ull << 31)) return bad(PIC_ERR_INVALID_ARG, "grid too large for 32-bit cell indices");
+  t.tvol = t.T[0] * t.T[1] * t.T[2];
+  t.key_mode = sort_key_mode;
+  if (n == 0) return PIC_OK;
+  if (!x || !y || !z || !cell || !perm) return bad(PIC_ERR_INVALID_ARG, "null particle or output array");
+  cudaError_t e = prec == PIC_F64
+                      ? sort_permutation_noalloc<double>(n_cells, dx, t, (const double*)x, (const double*)y, (const double*)z, n, cell,
+                                                         perm, (cudaStream_t)cuda_stream)
+                      : sort_permutation_noalloc<float>(n_cells, dx, t, (const float*)x, (const float*)y, (const float*)z, n, cell,
+                                                        perm, (cudaStream_t)cuda_stream);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return bad(PIC_ERR_CUDA, std::string("pic_sort_permutation_noalloc: ") + cudaGetErrorString(e));
+  }
+  return PIC_OK;
+}
